@@ -1,0 +1,373 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the cdmt hot path on B200 (contract: see DESIGN.md "Measurement").
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config c3] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (unpack + forward FFT + fused per-DM kernel, every
+block, every DM) over one synthetic observation of the named config.  Metric (BASELINE.json):
+input samples x DM trials per second = nsub * T * ndm / t.  One JSON line is printed by rank 0.
+
+N > 1 (torchrun): the path has no exchange step, so each rank runs its own observation of the
+same config (another beam: other seed) on its own GPU -- weak scaling, no data-path collective;
+torch.distributed is used for the barrier and the max-over-ranks of the device time only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1607_00909_b200 import synth  # noqa: E402
+
+METRIC = "input_samples_x_dm_trials_per_s"
+UNIT = "samples*DM/s"
+# FP32 (non-tensor) peak of a B200: 148 SMs x 128 FP32 lanes x 2 flop/FMA x 1.965 GHz
+# (unit counts and clocks: /opt/skills/guides/B200_PROFILING.md, MEASURED_PEAKS.json sm_max_mhz)
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+# DRAM bytes per fused-kernel launch from the committed ncu capture (profiles/); None until measured
+FUSED_TRAFFIC_BYTES_PER_LAUNCH = None
+
+
+def algorithmic_flops_per_unit_dm(cfg: synth.Config) -> float:
+    """SURVEY.md 8(d) / DESIGN.md: flops credited to one (subband, block) unit at one DM:
+    2 pols x C backward FFTs of M at 5 M log2 M, a complex multiply (6) on both pols per bin,
+    ~20 flops to form the chirp sample per bin, 8 per detected (kept) sample."""
+    N, C, M = cfg.nfft, cfg.nchan, cfg.mbin
+    V = M - 2 * cfg.half_discard
+    return 2 * C * 5.0 * M * np.log2(M) + 2 * 6.0 * N + 20.0 * N + 8.0 * C * V
+
+
+def shard_seed(seed: int, rank: int) -> int:
+    """Rank r processes its own observation: same recipe, another seed."""
+    return seed + 1000 * rank
+
+
+def rank_workload(cfg: synth.Config, rank: int, world: int) -> synth.Config:
+    """Weak scaling: every rank gets a full observation of the config (its own beam)."""
+    if world > 1:
+        cfg.seed = shard_seed(cfg.seed, rank)
+    return cfg
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [t.strip() for t in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(cfg: synth.Config, nunits: int, x_sub0: np.ndarray):
+    """Time the oracle, as it stands, on `nunits` (subband 0, block b) units with every DM."""
+    from oracle import cdmt_oracle as orc
+    p = orc.Params(**cfg.plan_kwargs())
+    blocks = np.stack([x_sub0[:, b * cfg.step:b * cfg.step + cfg.nfft] for b in range(nunits)])
+    t0 = time.perf_counter()
+    orc.units(p, [0] * nunits, blocks)
+    dt = time.perf_counter() - t0
+    samples_dm = nunits / float(cfg.nsub * cfg.nblock) * cfg.nsub * cfg.nsamp * cfg.ndm
+    return samples_dm / dt, dt, orc.num_threads()
+
+
+def run_reference(args, cfg, rank, world):
+    """--impl reference: the CPU oracle on the host cores, bounded sample per step."""
+    if rank != 0:
+        return
+    from oracle import cdmt_oracle as orc
+    ncores = orc.num_threads()
+    x0 = synth.generate_subband(cfg, 0)
+    nunits = min(cfg.nblock, max(1, ncores))
+    for _ in range(args.warmup):
+        oracle_sample(cfg, min(nunits, 2), x0)
+    t0 = time.perf_counter()
+    done = 0.0
+    for _ in range(args.steps):
+        rate, dt, _ = oracle_sample(cfg, nunits, x0)
+        done += rate * dt
+    total = time.perf_counter() - t0
+    value = done / total
+    sample = "%d of %d (subband, block) units of %s x all %d DMs per step" % (
+        nunits, cfg.nsub * cfg.nblock, cfg.name, cfg.ndm)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": total / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": workload_config(cfg, args),
+        "real_time_factor": value / (cfg.nsub * cfg.ndm) * synth.TSAMP_S,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": ncores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(cfg, args):
+    return {"workload": "%s: %d subbands x 2^%d samples, nfft=%d noverlap=%d nchan=%d ndec=%d, %d DM trials, %s in"
+            % (cfg.name, cfg.nsub, int(np.log2(cfg.nsamp)), cfg.nfft, cfg.noverlap, cfg.nchan, cfg.ndec,
+               cfg.ndm, "int8" if cfg.in_dtype == synth.IN_CI8 else "complex64"),
+            "nsub": cfg.nsub, "nsamp": cfg.nsamp, "nfft": cfg.nfft, "noverlap": cfg.noverlap,
+            "nchan": cfg.nchan, "ndec": cfg.ndec, "ndm": cfg.ndm, "nblock": cfg.nblock,
+            "parallelism": "replicas x%d (one observation per GPU, no collective)" % args.gpus,
+            "l2": "inputs (%.1f GB) and spectra exceed the 126 MB L2; no flush needed" % (
+                cfg.nsub * 2 * cfg.nsamp * (2 if cfg.in_dtype == synth.IN_CI8 else 8) / 1e9)}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="c3", choices=synth.CONFIG_NAMES)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--chunk-units", type=int, default=0)
+    ap.add_argument("--dm-tile", type=int, default=0)
+    ap.add_argument("--gen-threads", type=int, default=0)
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    cfg = rank_workload(synth.make_config(args.config), rank, world)
+
+    if args.impl == "reference":
+        run_reference(args, cfg, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_1607_00909_b200 import cdmt
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback for the product path")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    # ---- synthetic observation -> HBM (not timed)
+    nthreads = args.gen_threads or max(1, (os.cpu_count() or 1) // max(1, world))
+    int8 = cfg.in_dtype == synth.IN_CI8
+    if int8:
+        d_in = torch.empty((cfg.nsub, 2, cfg.nsamp, 2), dtype=torch.int8, device=dev)
+    else:
+        d_in = torch.empty((cfg.nsub, 2, cfg.nsamp), dtype=torch.complex64, device=dev)
+    want_e2e = not args.no_e2e
+    h_in = None
+    if want_e2e:
+        h_in = torch.empty(d_in.shape, dtype=d_in.dtype).pin_memory()
+    x_sub0 = None
+    from concurrent.futures import ThreadPoolExecutor
+    t_gen = time.perf_counter()
+    with ThreadPoolExecutor(nthreads) as ex:
+        for s, xs in zip(range(cfg.nsub), ex.map(lambda s: synth.generate_subband(cfg, s), range(cfg.nsub))):
+            if s == 0:
+                x_sub0 = xs
+            t = torch.from_numpy(xs)
+            if h_in is not None:
+                h_in[s].copy_(t)
+                d_in[s].copy_(h_in[s], non_blocking=True)
+            else:
+                d_in[s].copy_(t)
+    torch.cuda.synchronize()
+    t_gen = time.perf_counter() - t_gen
+
+    plan = cdmt.cdmt_plan_create(**cfg.plan_kwargs())
+    if args.chunk_units:
+        cdmt.cdmt_plan_set_option(plan, cdmt.OPT_CHUNK_UNITS, args.chunk_units)
+    if args.dm_tile:
+        cdmt.cdmt_plan_set_option(plan, cdmt.OPT_DM_TILE, args.dm_tile)
+    q = cdmt.cdmt_plan_query(plan, cfg.nsamp)
+    nch = cfg.nsub * cfg.nchan
+    nt = q["nout_per_chan"]
+    ws = torch.empty(q["workspace_bytes"], dtype=torch.uint8, device=dev)
+
+    # output: the whole filterbank set if it fits beside the rest, else block groups through one buffer
+    free_b, _ = torch.cuda.mem_get_info(dev)
+    out_bytes = q["out_bytes"]
+    groups = 1
+    while out_bytes / groups > 0.6 * free_b:
+        groups += 1
+    nb_total = q["nblock"]
+    nb_group = (nb_total + groups - 1) // groups
+    out = torch.empty((cfg.ndm, nb_group * cfg.nvalid_dec, nch), dtype=torch.float32, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        """One pass of the whole hot path over the observation (block groups share `out`)."""
+        launches = 0
+        b0 = 0
+        while b0 < nb_total:
+            nb = min(nb_group, nb_total - b0)
+            ns = (nb - 1) * cfg.step + cfg.nfft
+            off = b0 * cfg.step
+            esz = 2 if int8 else 8
+            cdmt.cdmt_execute(plan, d_in.data_ptr() + off * esz, ns, cfg.nsamp, out, out[0].numel(),
+                              ws, ws.numel(), stream)
+            launches += cdmt.cdmt_last_launch_count(plan)
+            b0 += nb
+        return launches
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+
+    # ---- timed region: K steps, device time, max over ranks
+    cdmt.cdmt_plan_set_option(plan, cdmt.OPT_PROFILE, 1)
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    torch.cuda.synchronize()
+    e0.record(stream)
+    launches = 0
+    for _ in range(args.steps):
+        launches += step()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    prof = cdmt.cdmt_profile_read(plan)
+    cdmt.cdmt_plan_set_option(plan, cdmt.OPT_PROFILE, 0)
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    sec_per_step = ms * 1e-3 / args.steps
+    samples_dm = float(cfg.nsub) * cfg.nsamp * cfg.ndm
+    value = world * samples_dm / sec_per_step
+
+    # ---- roofline of the dominant kernel (fused per-DM kernel): ALU bound
+    units_per_step = cfg.nsub * nb_total
+    flops_per_launch = algorithmic_flops_per_unit_dm(cfg) * cfg.ndm * units_per_step * args.steps / max(1, prof["n_fused"])
+    ms_per_launch = prof["ms_fused"] / max(1, prof["n_fused"])
+    achieved = flops_per_launch / (ms_per_launch * 1e-3) / 1e12
+    scratch = torch.empty(148 * 2 * 1024, dtype=torch.float32, device=dev)
+    fma_peak = cdmt.cdmt_measure_fp32_peak(scratch, scratch.numel() * 4, 3)
+    roofline = {"bound": "alu", "kernel": "k_fused", "achieved": achieved, "peak": FP32_PEAK_TFLOPS,
+                "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
+                "traffic": FUSED_TRAFFIC_BYTES_PER_LAUNCH,
+                "peak_source": "derived: 148 SM x 128 lanes x 2 x 1.965 GHz",
+                "fma_peak_measured_tflops": fma_peak,
+                "ms_per_launch": ms_per_launch, "launches_timed": prof["n_fused"],
+                "flops_per_launch": flops_per_launch,
+                "share_of_step": prof["ms_fused"] / ms,
+                "forward_fft_ms_per_step": prof["ms_forward"] / args.steps}
+
+    # ---- end to end through the host-buffer entry point (pinned host memory, copies timed)
+    e2e = None
+    if want_e2e:
+        del out
+        torch.cuda.empty_cache()
+        h_out = torch.empty((cfg.ndm, nt, nch), dtype=torch.float32).pin_memory()
+        nbytes = cdmt.cdmt_host_scratch_bytes(plan, cfg.nsamp)
+        d_scr = torch.empty(nbytes, dtype=torch.uint8, device=dev)
+        cdmt.cdmt_execute_host(plan, h_in.data_ptr(), cfg.nsamp, cfg.nsamp, h_out.data_ptr(), d_scr, nbytes, stream)
+        ksteps = max(1, min(args.steps, 3))
+        barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(ksteps):
+            cdmt.cdmt_execute_host(plan, h_in.data_ptr(), cfg.nsamp, cfg.nsamp, h_out.data_ptr(), d_scr, nbytes, stream)
+        torch.cuda.synchronize()
+        dt = (time.perf_counter() - t0) / ksteps
+        if world > 1:
+            t = torch.tensor([dt], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        esz = 2 if int8 else 8
+        e2e = {"value": world * samples_dm / dt, "unit": UNIT,
+               "h2d_bytes_per_step": int(cfg.nsub * 2 * q["nsamp_consumed"] * esz),
+               "d2h_bytes_per_step": int(q["out_bytes"]), "ms_per_step": dt * 1e3, "steps": ksteps,
+               "api": "cdmt_execute_host (pinned host in/out)"}
+        del d_scr
+
+    # ---- CPU baseline: the oracle, as it stands, on a bounded sample (rank 0, N=1 only)
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        from oracle import cdmt_oracle as orc
+        ncores = orc.num_threads()
+        nun = min(cfg.nblock, max(1, ncores))
+        rate, dt, ncores = oracle_sample(cfg, nun, x_sub0)
+        cpu = {"value": rate, "unit": UNIT, "cores": ncores, "kind": "oracle", "seconds": dt,
+               "sample": "%d of %d (subband, block) units of %s x all %d DMs" % (
+                   nun, cfg.nsub * cfg.nblock, cfg.name, cfg.ndm)}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": sec_per_step * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": workload_config(cfg, args),
+            "real_time_factor": cfg.nsamp * synth.TSAMP_S / sec_per_step,
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+            "roofline": roofline, "cpu_baseline": cpu,
+            "gen_seconds": t_gen, "out_groups": groups,
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,179 @@
+/*
+ * cdmt.h -- C ABI of the B200-native coherent-dedispersion hot path
+ * (Bassa, Pleunis & Hessels, arXiv:1607.00909, "cdmt"; line numbers below are PAPER.md).
+ *
+ * What the library computes (Fig. 2; Algorithm 1), for every
+ * subband s < nsub, overlap-save block b < nblock, channel c < nchan and DM trial d < ndm:
+ *
+ *   step = nfft - noverlap, M = nfft/nchan, h = noverlap/(2 nchan), Vd = (M - 2h)/ndec
+ *   u_p[n]  = in[s][p][b step + n],                 n < nfft, p < 2       (l.95)
+ *   U_p[k]  = sum_n u_p[n] exp(-2 pi i k n / nfft)                         (l.96)
+ *   Xs_p[j] = U_p[(j + nfft/2) mod nfft]            bins in increasing frequency   (l.97)
+ *   Z_p[m]  = Xs_p[c M + m] exp(+2 pi i dm[d] f^2 / (2.41e-10 f0^2 (f0 + f)))   (l.99; Eq. 1)
+ *             f0, f in MHz: CDMT_REF_CHANNEL f0 = centre of channel c, f = (m - M/2) bw/nfft
+ *                           CDMT_REF_SUBBAND f0 = fcen[s], f = (c M + m - nfft/2) bw/nfft
+ *   y_p[t]  = sum_m Z_p[m] exp(+2 pi i (m - M/2) t / M),  t < M            (l.101-102)
+ *   I[t]    = (|y_0[t]|^2 + |y_1[t]|^2) / (nfft M)                         (l.103)
+ *   out[d][b Vd + q][nsub nchan - 1 - (s nchan + c)] = sum_{r<ndec} I[h + q ndec + r]
+ *
+ * i.e. one float32 filterbank per DM, time-major, channel-fastest, DECREASING frequency
+ * (PAPER.md:123).  Blocks are "valid only": nblock = floor((nsamp - nfft)/step) + 1, the first
+ * output sample starts at input sample noverlap/2, trailing samples that do not fill a block
+ * are ignored.
+ *
+ * Conventions
+ *  - Pointers named d_* are DEVICE pointers, h_* are HOST pointers.  The caller owns all of
+ *    them; the library never allocates device memory.  A plan owns only host state.
+ *  - Every entry point returns a CDMT_* status and never aborts or throws.  All arguments
+ *    are validated on the host before anything is launched.
+ *  - cdmt_execute and the stage calls are asynchronous on `cuda_stream` (a cudaStream_t
+ *    passed as void*; NULL = the legacy default stream) and do no host synchronisation.
+ *    They are stateless between calls; one call may be in flight per (plan, workspace).
+ */
+#ifndef CDMT_H
+#define CDMT_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cdmt_plan cdmt_plan; /* opaque */
+
+enum {
+    CDMT_OK = 0,
+    CDMT_ERR_ARG = 1,       /* null / misaligned pointer, non-finite or non-positive value */
+    CDMT_ERR_SIZE = 2,      /* sizes violate a divisibility / range rule listed below */
+    CDMT_ERR_WORKSPACE = 3, /* workspace_bytes smaller than cdmt_plan_query reports */
+    CDMT_ERR_CUDA = 4,      /* a CUDA call or launch failed (sticky error cleared) */
+    CDMT_ERR_ALLOC = 5      /* host allocation failed */
+};
+
+enum { CDMT_IN_CF32 = 0, CDMT_IN_CI8 = 1 };          /* interleaved (re, im) float32 / int8 */
+enum { CDMT_REF_CHANNEL = 0, CDMT_REF_SUBBAND = 1 }; /* nu_0 of Eq. 1 */
+
+/* Tuning knobs for cdmt_plan_set_option (defaults chosen by the library). */
+enum {
+    CDMT_OPT_CHUNK_UNITS = 0, /* (subband, block) units whose spectra are resident at once */
+    CDMT_OPT_DM_TILE = 1,     /* DM trials looped inside one CTA of the fused kernel (0 = all) */
+    CDMT_OPT_ACCURATE_SINCOS = 2, /* 1: sincospif instead of the fast approximation */
+    CDMT_OPT_PROFILE = 3      /* 1: record CUDA events round each kernel class (cdmt_profile_read) */
+};
+
+/*
+ * Create a plan ("user-defined choices" n_c, N_bin, n_d and the DM list).
+ *   nsub      number of subbands (>= 1)
+ *   fcen_mhz  HOST [nsub] subband centre frequencies in MHz, ascending; copied
+ *   bw_mhz    subband bandwidth = complex sample rate, MHz (> 0; fcen - bw/2 > 0)
+ *   nfft      N_bin, power of two, 256 <= nfft <= 2^20
+ *   noverlap  n_d n_c in INPUT samples: 0 <= noverlap < nfft, noverlap % (2 nchan) == 0
+ *   nchan     n_c, power of two, 16 <= nfft/nchan <= 16384
+ *   ndec      time-integration factor >= 1, (nfft - noverlap) % (nchan ndec) == 0
+ *   ndm, dm   HOST [ndm] DM trials in pc cm^-3 (any sign: -DM applies the conjugate chirp); copied
+ *   in_dtype  CDMT_IN_*; chirp_ref CDMT_REF_*
+ * Errors: CDMT_ERR_ARG, CDMT_ERR_SIZE, CDMT_ERR_ALLOC.  *plan is NULL on error.
+ * Pure host code: works without a GPU.
+ */
+int cdmt_plan_create(cdmt_plan **plan, int nsub, const double *fcen_mhz, double bw_mhz,
+                     int nfft, int noverlap, int nchan, int ndec, int ndm, const double *dm,
+                     int in_dtype, int chirp_ref);
+
+int cdmt_plan_destroy(cdmt_plan *plan);
+
+/* Set a CDMT_OPT_* knob; CDMT_ERR_ARG for an unknown key or out-of-range value. */
+int cdmt_plan_set_option(cdmt_plan *plan, int key, long long value);
+
+/*
+ * Sizes for an input of `nsamp` samples per polarisation per subband (host arithmetic only;
+ * PAPER.md:81, 123).  Any output pointer may be NULL.
+ *   nblock          blocks processed
+ *   nsamp_consumed  (nblock-1) step + nfft: samples actually read
+ *   nout_per_chan   nblock * Vd output time samples per channel per DM
+ *   out_bytes       ndm * nout_per_chan * nsub*nchan * 4 (dense DM planes)
+ *   workspace_bytes bytes cdmt_execute needs in d_workspace
+ * Errors: CDMT_ERR_ARG (null plan), CDMT_ERR_SIZE (nsamp < nfft).
+ */
+int cdmt_plan_query(const cdmt_plan *plan, long long nsamp, int *nblock,
+                    long long *nsamp_consumed, long long *nout_per_chan, size_t *out_bytes,
+                    size_t *workspace_bytes);
+
+/*
+ * Run the whole hot path on device-resident input.
+ *   d_in           DEVICE, [nsub][2 pols][..] complex words of the plan's in_dtype, time
+ *                  fastest; row (s, p) starts at element (2 s + p) * in_stride_pol.
+ *                  16-byte aligned.
+ *   nsamp          samples per row to process (>= nfft)
+ *   in_stride_pol  distance between consecutive rows, in complex samples (>= nsamp; even for
+ *                  CDMT_IN_CF32 so that every row is 16-byte aligned)
+ *   d_out          DEVICE float32, DM plane d starts at d * out_stride_dm elements; inside a
+ *                  plane [nblock*Vd][nsub*nchan].  Every element of every plane is written.
+ *   out_stride_dm  elements between DM planes (>= nblock*Vd*nsub*nchan)
+ *   d_workspace    DEVICE scratch, 256-byte aligned, >= workspace_bytes from cdmt_plan_query
+ *   cuda_stream    cudaStream_t
+ * To stream a long observation call repeatedly, advancing d_in by nblock*step samples (the
+ * last noverlap samples are re-supplied).
+ * Errors: CDMT_ERR_ARG, CDMT_ERR_SIZE, CDMT_ERR_WORKSPACE, CDMT_ERR_CUDA.
+ */
+int cdmt_execute(cdmt_plan *plan, const void *d_in, long long nsamp, long long in_stride_pol,
+                 float *d_out, long long out_stride_dm, void *d_workspace,
+                 size_t workspace_bytes, void *cuda_stream);
+
+/*
+ * The same path with HOST buffers (read block, copy to device, ...,
+ * copy to host).  h_in / h_out have the layouts of d_in / d_out (h_out planes dense:
+ * stride nblock*Vd*nsub*nchan) and should be pinned for full copy speed.  The caller lends
+ * device scratch `d_scratch` of at least cdmt_host_scratch_bytes(); input, workspace and
+ * output are staged there in groups of blocks.  Copies and kernels are issued on
+ * `cuda_stream`; the call returns after the last device-to-host copy has completed.
+ */
+int cdmt_execute_host(cdmt_plan *plan, const void *h_in, long long nsamp,
+                      long long in_stride_pol, float *h_out, void *d_scratch,
+                      size_t scratch_bytes, void *cuda_stream);
+int cdmt_host_scratch_bytes(const cdmt_plan *plan, long long nsamp, size_t *scratch_bytes);
+
+/*
+ * Stage entry points (used by the per-kernel parity tests; same validation rules).
+ *
+ * cdmt_unpack: Alg. 1 l.95 "unpack, segment and pad": writes the overlapped
+ * blocks as float32 complex, d_blocks[(b nsub + s)][p][nfft].
+ *
+ * cdmt_forward_spectrum: l.95-97: unpack + forward FFT + swap halves; d_spec[(b nsub + s)][p][nfft]
+ * holds Xs_p[j] (float32 complex, increasing frequency).  Needs the same workspace as cdmt_execute.
+ */
+int cdmt_unpack(cdmt_plan *plan, const void *d_in, long long nsamp, long long in_stride_pol,
+                void *d_blocks, void *cuda_stream);
+int cdmt_forward_spectrum(cdmt_plan *plan, const void *d_in, long long nsamp,
+                          long long in_stride_pol, void *d_spec, void *d_workspace,
+                          size_t workspace_bytes, void *cuda_stream);
+
+/* Eq. 2: dispersion sweep across [fcen - bw/2, fcen + bw/2] in seconds. */
+double cdmt_sweep_seconds(double fcen_mhz, double bw_mhz, double dm);
+/* smallest legal noverlap (input samples, rounded up to a multiple of 2 nchan)
+ * that covers the sweep of the lowest channel (REF_CHANNEL) or lowest subband (REF_SUBBAND)
+ * at the largest |DM| of the plan. */
+long long cdmt_min_overlap(const cdmt_plan *plan);
+
+/* Measure the FP32 FMA rate of the device the stream belongs to (the "alu" roofline
+ * denominator): runs `iters` dependent-chain FMA launches and returns
+ * TFLOP/s in *tflops.  d_scratch: >= 4 bytes * 148 * 1024. */
+int cdmt_measure_fp32_peak(void *d_scratch, size_t scratch_bytes, int iters, double *tflops,
+                           void *cuda_stream);
+
+/* With CDMT_OPT_PROFILE = 1 every execute records CUDA events on its stream round (kind 0) the
+ * two forward-FFT passes of a chunk and (kind 1) each fused per-DM kernel launch.  This call
+ * waits for the recorded events, returns the summed durations in milliseconds and the number of
+ * spans of each kind since the previous read, and resets the record. */
+int cdmt_profile_read(cdmt_plan *plan, double *ms_forward, double *ms_fused,
+                      long long *n_forward, long long *n_fused);
+
+/* Number of kernel launches cdmt_execute issued on its last call with this plan. */
+long long cdmt_last_launch_count(const cdmt_plan *plan);
+
+const char *cdmt_strerror(int status);
+const char *cdmt_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CDMT_H */

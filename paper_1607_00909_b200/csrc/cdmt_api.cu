@@ -1,0 +1,468 @@
+// cdmt_api.cu -- the C ABI declared in include/cdmt.h: plan bookkeeping (host only) and the
+// launch sequences.  No arithmetic of the method lives here except the Eq. 2 helper.
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/cdmt.h"
+#include "cdmt_internal.h"
+
+using namespace cdmt;
+
+struct cdmt_plan {
+    Geometry g;
+    std::vector<double> fcen, dm;
+    long long chunk_units;   // 0 = automatic
+    int dm_tile;             // 0 = all
+    int accurate;
+    int profile;             // record CUDA events around each kernel class
+    long long last_launches;
+    std::vector<cudaEvent_t> ev_pool;   // created lazily, reused
+    size_t ev_used;
+    struct Span { size_t e0, e1; int kind; };   // kind 0: forward FFT passes, 1: fused per-DM kernel
+    std::vector<Span> spans;
+};
+
+static cudaEvent_t plan_event(cdmt_plan *p, size_t *idx)
+{
+    if (p->ev_used == p->ev_pool.size()) {
+        cudaEvent_t e = nullptr;
+        if (cudaEventCreate(&e) != cudaSuccess) return nullptr;
+        p->ev_pool.push_back(e);
+    }
+    *idx = p->ev_used;
+    return p->ev_pool[p->ev_used++];
+}
+
+static bool is_pow2(long long x) { return x > 0 && (x & (x - 1)) == 0; }
+
+static int ilog2(long long x)
+{
+    int n = 0;
+    while ((1LL << n) < x) ++n;
+    return n;
+}
+
+extern "C" const char *cdmt_strerror(int status)
+{
+    switch (status) {
+    case CDMT_OK: return "ok";
+    case CDMT_ERR_ARG: return "invalid argument (null or misaligned pointer, or bad value)";
+    case CDMT_ERR_SIZE: return "sizes violate a divisibility or range rule";
+    case CDMT_ERR_WORKSPACE: return "workspace too small";
+    case CDMT_ERR_CUDA: return "CUDA call or kernel launch failed";
+    case CDMT_ERR_ALLOC: return "host allocation failed";
+    default: return "unknown status";
+    }
+}
+
+extern "C" const char *cdmt_version(void) { return "cdmt-b200 0.1 (sm_100a)"; }
+
+// Eq. 2.
+extern "C" double cdmt_sweep_seconds(double fcen_mhz, double bw_mhz, double dm)
+{
+    const double lo = fcen_mhz - 0.5 * bw_mhz, hi = fcen_mhz + 0.5 * bw_mhz;
+    return (1.0 / 2.41e-4) * (1.0 / (lo * lo) - 1.0 / (hi * hi)) * dm;
+}
+
+extern "C" int cdmt_plan_create(cdmt_plan **plan, int nsub, const double *fcen_mhz, double bw_mhz, int nfft,
+                                int noverlap, int nchan, int ndec, int ndm, const double *dm, int in_dtype,
+                                int chirp_ref)
+{
+    if (!plan) return CDMT_ERR_ARG;
+    *plan = nullptr;
+    if (!fcen_mhz || !dm || nsub < 1 || ndm < 1) return CDMT_ERR_ARG;
+    if (!(bw_mhz > 0.0) || !std::isfinite(bw_mhz)) return CDMT_ERR_ARG;
+    if (in_dtype != CDMT_IN_CF32 && in_dtype != CDMT_IN_CI8) return CDMT_ERR_ARG;
+    if (chirp_ref != CDMT_REF_CHANNEL && chirp_ref != CDMT_REF_SUBBAND) return CDMT_ERR_ARG;
+    for (int s = 0; s < nsub; ++s)
+        if (!std::isfinite(fcen_mhz[s]) || !(fcen_mhz[s] - 0.5 * bw_mhz > 0.0)) return CDMT_ERR_ARG;
+    for (int d = 0; d < ndm; ++d)
+        if (!std::isfinite(dm[d])) return CDMT_ERR_ARG;
+    if (!is_pow2(nfft) || nfft < 256 || nfft > (1 << 20)) return CDMT_ERR_SIZE;
+    if (!is_pow2(nchan) || nchan > nfft) return CDMT_ERR_SIZE;
+    const int M = nfft / nchan;
+    if (!fused_len_supported(M)) return CDMT_ERR_SIZE;
+    if (ndec < 1) return CDMT_ERR_SIZE;
+    if (noverlap < 0 || noverlap >= nfft || noverlap % (2 * nchan) != 0) return CDMT_ERR_SIZE;
+    if ((nfft - noverlap) % (nchan * ndec) != 0) return CDMT_ERR_SIZE;
+
+    cdmt_plan *p = new (std::nothrow) cdmt_plan();
+    if (!p) return CDMT_ERR_ALLOC;
+    try {
+        p->fcen.assign(fcen_mhz, fcen_mhz + nsub);
+        p->dm.assign(dm, dm + ndm);
+    } catch (...) {
+        delete p;
+        return CDMT_ERR_ALLOC;
+    }
+    Geometry &g = p->g;
+    g.nsub = nsub; g.nfft = nfft; g.noverlap = noverlap; g.nchan = nchan; g.ndec = ndec; g.ndm = ndm;
+    g.in_dtype = in_dtype; g.chirp_ref = chirp_ref; g.bw_mhz = bw_mhz;
+    g.step = nfft - noverlap;
+    g.mbin = M;
+    g.hdisc = noverlap / (2 * nchan);
+    g.vdec = (M - 2 * g.hdisc) / ndec;
+    const int lg = ilog2(nfft);
+    g.n1 = 1 << ((lg + 1) / 2);
+    g.n2 = nfft / g.n1;
+    g.lo_bits = (lg + 1) / 2;
+    g.tw_hi_bits = lg - g.lo_bits;
+    if (!forward_len_supported(g.n1) || !forward_len_supported(g.n2)) {
+        delete p;
+        return CDMT_ERR_SIZE;
+    }
+    p->chunk_units = 0;
+    p->dm_tile = 0;
+    p->accurate = 0;
+    p->profile = 0;
+    p->ev_used = 0;
+    p->last_launches = 0;
+    *plan = p;
+    return CDMT_OK;
+}
+
+extern "C" int cdmt_plan_destroy(cdmt_plan *plan)
+{
+    if (!plan) return CDMT_ERR_ARG;
+    for (cudaEvent_t e : plan->ev_pool) cudaEventDestroy(e);
+    delete plan;
+    return CDMT_OK;
+}
+
+extern "C" int cdmt_plan_set_option(cdmt_plan *plan, int key, long long value)
+{
+    if (!plan) return CDMT_ERR_ARG;
+    switch (key) {
+    case CDMT_OPT_CHUNK_UNITS:
+        if (value < 0 || value > (1 << 30)) return CDMT_ERR_ARG;
+        plan->chunk_units = value;
+        return CDMT_OK;
+    case CDMT_OPT_DM_TILE:
+        if (value < 0 || value > (1 << 30)) return CDMT_ERR_ARG;
+        plan->dm_tile = (int)value;
+        return CDMT_OK;
+    case CDMT_OPT_ACCURATE_SINCOS:
+        if (value != 0 && value != 1) return CDMT_ERR_ARG;
+        plan->accurate = (int)value;
+        return CDMT_OK;
+    case CDMT_OPT_PROFILE:
+        if (value != 0 && value != 1) return CDMT_ERR_ARG;
+        plan->profile = (int)value;
+        return CDMT_OK;
+    default: return CDMT_ERR_ARG;
+    }
+}
+
+static long long nblock_for(const Geometry &g, long long nsamp)
+{
+    return nsamp < g.nfft ? 0 : (nsamp - g.nfft) / g.step + 1;
+}
+
+// units resident at once: by default about 1 GiB of spectra
+static long long chunk_units_for(const cdmt_plan *p, long long nunits)
+{
+    long long c = p->chunk_units;
+    if (c <= 0) {
+        const long long per_unit = 2LL * p->g.nfft * (long long)sizeof(float2);
+        c = (1LL << 30) / per_unit;
+        if (c < 1) c = 1;
+    }
+    // grid.x of the fused kernel = chunk * nchan must stay below 2^31
+    const long long cap = ((1LL << 31) - 1) / p->g.nchan / 2;
+    if (c > cap) c = cap;
+    if (c > nunits) c = nunits;
+    return c < 1 ? 1 : c;
+}
+
+extern "C" int cdmt_plan_query(const cdmt_plan *plan, long long nsamp, int *nblock, long long *nsamp_consumed,
+                               long long *nout_per_chan, size_t *out_bytes, size_t *workspace_bytes)
+{
+    if (!plan) return CDMT_ERR_ARG;
+    const Geometry &g = plan->g;
+    const long long nb = nblock_for(g, nsamp);
+    if (nb < 1 || nb > (1LL << 30)) return CDMT_ERR_SIZE;
+    if (nblock) *nblock = (int)nb;
+    if (nsamp_consumed) *nsamp_consumed = (nb - 1) * g.step + g.nfft;
+    if (nout_per_chan) *nout_per_chan = nb * g.vdec;
+    if (out_bytes) *out_bytes = (size_t)g.ndm * (size_t)(nb * g.vdec) * (size_t)g.nsub * g.nchan * sizeof(float);
+    if (workspace_bytes) {
+        const long long cu = chunk_units_for(plan, nb * g.nsub);
+        *workspace_bytes = workspace_layout(g, (int)cu, nullptr, nullptr);
+    }
+    return CDMT_OK;
+}
+
+static int check_cuda(cudaError_t e)
+{
+    if (e == cudaSuccess) return CDMT_OK;
+    cudaGetLastError();  // clear the sticky state
+    return CDMT_ERR_CUDA;
+}
+
+static int validate_input(const cdmt_plan *plan, const void *d_in, long long nsamp, long long in_stride_pol,
+                          long long *nb)
+{
+    if (!plan || !d_in) return CDMT_ERR_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_in) & 15) != 0) return CDMT_ERR_ARG;
+    const Geometry &g = plan->g;
+    if (nsamp < g.nfft) return CDMT_ERR_SIZE;
+    if (in_stride_pol < nsamp) return CDMT_ERR_SIZE;
+    // float32 rows are read with 16-byte vector loads: the row stride must be even
+    if (g.in_dtype == CDMT_IN_CF32 && (in_stride_pol & 1)) return CDMT_ERR_SIZE;
+    *nb = nblock_for(g, nsamp);
+    if (*nb < 1 || *nb * g.nsub > (1LL << 30)) return CDMT_ERR_SIZE;
+    return CDMT_OK;
+}
+
+static int run_chunks(cdmt_plan *plan, const void *d_in, long long in_stride_pol, long long nb, float *d_out,
+                      long long out_stride_dm, float2 *d_spec_out, void *d_workspace, size_t workspace_bytes,
+                      cudaStream_t st)
+{
+    const Geometry &g = plan->g;
+    const long long nunits = nb * g.nsub;
+    const long long cu = chunk_units_for(plan, nunits);
+    Workspace ws;
+    const size_t need = workspace_layout(g, (int)cu, reinterpret_cast<char *>(d_workspace), &ws);
+    if (workspace_bytes < need) return CDMT_ERR_WORKSPACE;
+    plan->last_launches = 0;
+    int rc = check_cuda(launch_init_tables(g, ws, plan->dm.data(), plan->fcen.data(), st, &plan->last_launches));
+    if (rc) return rc;
+    auto mark = [&](size_t *idx) -> bool {
+        if (!plan->profile) return true;
+        cudaEvent_t e = plan_event(plan, idx);
+        return e && cudaEventRecord(e, st) == cudaSuccess;
+    };
+    for (long long u0 = 0; u0 < nunits; u0 += cu) {
+        const int n = (int)((nunits - u0 < cu) ? nunits - u0 : cu);
+        float2 *spec = d_spec_out ? d_spec_out + (size_t)u0 * 2 * g.nfft : ws.spec;
+        size_t a = 0, b = 0, c = 0;
+        if (!mark(&a)) return check_cuda(cudaErrorUnknown);
+        rc = check_cuda(launch_forward(g, ws, d_in, in_stride_pol, (int)u0, n, spec, st, &plan->last_launches));
+        if (rc) return rc;
+        if (!mark(&b)) return check_cuda(cudaErrorUnknown);
+        if (plan->profile) plan->spans.push_back({a, b, 0});
+        if (d_out) {
+            rc = check_cuda(launch_fused(g, ws, spec, (int)u0, n, d_out, out_stride_dm, plan->dm_tile,
+                                         plan->accurate, st, &plan->last_launches));
+            if (rc) return rc;
+            if (!mark(&c)) return check_cuda(cudaErrorUnknown);
+            if (plan->profile) plan->spans.push_back({b, c, 1});
+        }
+    }
+    return CDMT_OK;
+}
+
+// Sum of the event-timed kernel durations recorded since the last read (CDMT_OPT_PROFILE = 1).
+// Synchronises on the recorded events.
+extern "C" int cdmt_profile_read(cdmt_plan *plan, double *ms_forward, double *ms_fused, long long *n_forward,
+                                 long long *n_fused)
+{
+    if (!plan) return CDMT_ERR_ARG;
+    double t[2] = {0.0, 0.0};
+    long long n[2] = {0, 0};
+    int rc = CDMT_OK;
+    for (const cdmt_plan::Span &sp : plan->spans) {
+        float ms = 0.f;
+        if (cudaEventSynchronize(plan->ev_pool[sp.e1]) != cudaSuccess ||
+            cudaEventElapsedTime(&ms, plan->ev_pool[sp.e0], plan->ev_pool[sp.e1]) != cudaSuccess) {
+            rc = check_cuda(cudaErrorUnknown);
+            break;
+        }
+        t[sp.kind] += ms;
+        n[sp.kind] += 1;
+    }
+    plan->spans.clear();
+    plan->ev_used = 0;
+    if (ms_forward) *ms_forward = t[0];
+    if (ms_fused) *ms_fused = t[1];
+    if (n_forward) *n_forward = n[0];
+    if (n_fused) *n_fused = n[1];
+    return rc;
+}
+
+extern "C" int cdmt_execute(cdmt_plan *plan, const void *d_in, long long nsamp, long long in_stride_pol,
+                            float *d_out, long long out_stride_dm, void *d_workspace, size_t workspace_bytes,
+                            void *cuda_stream)
+{
+    long long nb = 0;
+    int rc = validate_input(plan, d_in, nsamp, in_stride_pol, &nb);
+    if (rc) return rc;
+    if (!d_out || !d_workspace) return CDMT_ERR_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_workspace) & 255) != 0) return CDMT_ERR_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_out) & 3) != 0) return CDMT_ERR_ARG;
+    const Geometry &g = plan->g;
+    if (out_stride_dm < nb * g.vdec * (long long)g.nsub * g.nchan) return CDMT_ERR_SIZE;
+    return run_chunks(plan, d_in, in_stride_pol, nb, d_out, out_stride_dm, nullptr, d_workspace, workspace_bytes,
+                      static_cast<cudaStream_t>(cuda_stream));
+}
+
+extern "C" int cdmt_forward_spectrum(cdmt_plan *plan, const void *d_in, long long nsamp, long long in_stride_pol,
+                                     void *d_spec, void *d_workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    long long nb = 0;
+    int rc = validate_input(plan, d_in, nsamp, in_stride_pol, &nb);
+    if (rc) return rc;
+    if (!d_spec || !d_workspace) return CDMT_ERR_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_workspace) & 255) != 0) return CDMT_ERR_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_spec) & 15) != 0) return CDMT_ERR_ARG;
+    return run_chunks(plan, d_in, in_stride_pol, nb, nullptr, 0, reinterpret_cast<float2 *>(d_spec), d_workspace,
+                      workspace_bytes, static_cast<cudaStream_t>(cuda_stream));
+}
+
+extern "C" int cdmt_unpack(cdmt_plan *plan, const void *d_in, long long nsamp, long long in_stride_pol,
+                           void *d_blocks, void *cuda_stream)
+{
+    long long nb = 0;
+    int rc = validate_input(plan, d_in, nsamp, in_stride_pol, &nb);
+    if (rc) return rc;
+    if (!d_blocks || (reinterpret_cast<uintptr_t>(d_blocks) & 15) != 0) return CDMT_ERR_ARG;
+    plan->last_launches = 0;
+    return check_cuda(launch_unpack(plan->g, d_in, in_stride_pol, (int)nb, reinterpret_cast<float2 *>(d_blocks),
+                                    static_cast<cudaStream_t>(cuda_stream), &plan->last_launches));
+}
+
+// ---- host-buffer path --------------------------------------------------------------------
+// blocks per staged group: keep the staged output near 1 GiB
+static long long host_group_blocks(const cdmt_plan *plan, long long nb)
+{
+    const Geometry &g = plan->g;
+    const long long per_block = (long long)g.ndm * g.vdec * g.nsub * g.nchan * (long long)sizeof(float);
+    long long gb = (1LL << 30) / (per_block > 0 ? per_block : 1);
+    if (gb < 1) gb = 1;
+    if (gb > nb) gb = nb;
+    return gb;
+}
+
+struct HostLayout {
+    size_t in_off, in_bytes, ws_off, ws_bytes, out_off, out_bytes, total;
+    long long gb, in_rowlen;
+};
+
+static int host_layout(const cdmt_plan *plan, long long nsamp, HostLayout *L)
+{
+    const Geometry &g = plan->g;
+    const long long nb = nblock_for(g, nsamp);
+    if (nb < 1) return CDMT_ERR_SIZE;
+    const long long esz = g.in_dtype == CDMT_IN_CI8 ? 2 : 8;
+    L->gb = host_group_blocks(plan, nb);
+    long long rowlen = (L->gb - 1) * g.step + g.nfft;
+    rowlen = (rowlen + 7) & ~7LL;  // keep rows 16-byte aligned for both word sizes
+    L->in_rowlen = rowlen;
+    auto al = [](size_t x) { return (x + 255) & ~(size_t)255; };
+    L->in_off = 0;
+    L->in_bytes = al((size_t)rowlen * esz * 2 * g.nsub);
+    L->ws_off = L->in_off + L->in_bytes;
+    const long long cu = chunk_units_for(plan, L->gb * g.nsub);
+    L->ws_bytes = al(workspace_layout(g, (int)cu, nullptr, nullptr));
+    L->out_off = L->ws_off + L->ws_bytes;
+    L->out_bytes = al((size_t)g.ndm * L->gb * g.vdec * g.nsub * g.nchan * sizeof(float));
+    L->total = L->out_off + L->out_bytes;
+    return CDMT_OK;
+}
+
+extern "C" int cdmt_host_scratch_bytes(const cdmt_plan *plan, long long nsamp, size_t *scratch_bytes)
+{
+    if (!plan || !scratch_bytes) return CDMT_ERR_ARG;
+    HostLayout L;
+    int rc = host_layout(plan, nsamp, &L);
+    if (rc) return rc;
+    *scratch_bytes = L.total;
+    return CDMT_OK;
+}
+
+extern "C" int cdmt_execute_host(cdmt_plan *plan, const void *h_in, long long nsamp, long long in_stride_pol,
+                                 float *h_out, void *d_scratch, size_t scratch_bytes, void *cuda_stream)
+{
+    if (!plan || !h_in || !h_out || !d_scratch) return CDMT_ERR_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_scratch) & 255) != 0) return CDMT_ERR_ARG;
+    const Geometry &g = plan->g;
+    if (nsamp < g.nfft || in_stride_pol < nsamp) return CDMT_ERR_SIZE;
+    HostLayout L;
+    int rc = host_layout(plan, nsamp, &L);
+    if (rc) return rc;
+    if (scratch_bytes < L.total) return CDMT_ERR_WORKSPACE;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const long long nb = nblock_for(g, nsamp);
+    const long long esz = g.in_dtype == CDMT_IN_CI8 ? 2 : 8;
+    char *base = reinterpret_cast<char *>(d_scratch);
+    char *d_in = base + L.in_off;
+    float *d_out = reinterpret_cast<float *>(base + L.out_off);
+    const size_t nchtot = (size_t)g.nsub * g.nchan;
+    const size_t plane_host = (size_t)nb * g.vdec * nchtot;
+    long long launches = 0;
+    for (long long b0 = 0; b0 < nb; b0 += L.gb) {
+        const long long nbg = (nb - b0 < L.gb) ? nb - b0 : L.gb;
+        const long long len = (nbg - 1) * g.step + g.nfft;
+        rc = check_cuda(cudaMemcpy2DAsync(d_in, (size_t)L.in_rowlen * esz,
+                                          reinterpret_cast<const char *>(h_in) + (size_t)b0 * g.step * esz,
+                                          (size_t)in_stride_pol * esz, (size_t)len * esz, (size_t)2 * g.nsub,
+                                          cudaMemcpyHostToDevice, st));
+        if (rc) return rc;
+        const size_t plane_dev = (size_t)nbg * g.vdec * nchtot;
+        rc = run_chunks(plan, d_in, L.in_rowlen, nbg, d_out, (long long)plane_dev, nullptr, base + L.ws_off,
+                        L.ws_bytes, st);
+        if (rc) return rc;
+        launches += plan->last_launches;
+        rc = check_cuda(cudaMemcpy2DAsync(h_out + (size_t)b0 * g.vdec * nchtot, plane_host * sizeof(float), d_out,
+                                          plane_dev * sizeof(float), plane_dev * sizeof(float), (size_t)g.ndm,
+                                          cudaMemcpyDeviceToHost, st));
+        if (rc) return rc;
+    }
+    plan->last_launches = launches;
+    return check_cuda(cudaStreamSynchronize(st));
+}
+
+// n_d n_c >= r t_d for the lowest-frequency channel (or subband) at the largest |DM|.
+extern "C" long long cdmt_min_overlap(const cdmt_plan *plan)
+{
+    if (!plan) return -1;
+    const Geometry &g = plan->g;
+    double dmax = 0.0;
+    for (double d : plan->dm) dmax = std::fabs(d) > dmax ? std::fabs(d) : dmax;
+    double fmin = plan->fcen[0];
+    for (double f : plan->fcen) fmin = f < fmin ? f : fmin;
+    double td;
+    if (g.chirp_ref == CDMT_REF_CHANNEL) {
+        const double cw = g.bw_mhz / g.nchan;
+        td = cdmt_sweep_seconds(fmin - 0.5 * g.bw_mhz + 0.5 * cw, cw, dmax);
+    } else {
+        td = cdmt_sweep_seconds(fmin, g.bw_mhz, dmax);
+    }
+    const long long samples = (long long)std::ceil(td * g.bw_mhz * 1e6);
+    const long long q = 2LL * g.nchan;
+    return (samples + q - 1) / q * q;
+}
+
+extern "C" long long cdmt_last_launch_count(const cdmt_plan *plan) { return plan ? plan->last_launches : -1; }
+
+extern "C" int cdmt_measure_fp32_peak(void *d_scratch, size_t scratch_bytes, int iters, double *tflops,
+                                      void *cuda_stream)
+{
+    if (!d_scratch || !tflops || iters < 1) return CDMT_ERR_ARG;
+    const int nblocks = 148 * 2, inner = 4096;
+    if (scratch_bytes < sizeof(float) * (size_t)nblocks * 1024) return CDMT_ERR_WORKSPACE;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    cudaEvent_t e0, e1;
+    if (check_cuda(cudaEventCreate(&e0)) || check_cuda(cudaEventCreate(&e1))) return CDMT_ERR_CUDA;
+    int rc = check_cuda(launch_fp32_peak(reinterpret_cast<float *>(d_scratch), nblocks, 64, st));  // warm-up
+    double best = 0.0;
+    for (int i = 0; i < iters && !rc; ++i) {
+        cudaEventRecord(e0, st);
+        rc = check_cuda(launch_fp32_peak(reinterpret_cast<float *>(d_scratch), nblocks, inner, st));
+        cudaEventRecord(e1, st);
+        if (rc) break;
+        rc = check_cuda(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double flops = (double)nblocks * 1024.0 * inner * 16.0 * 8.0 * 2.0;
+        const double tf = flops / (ms * 1e-3) * 1e-12;
+        if (tf > best) best = tf;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    *tflops = best;
+    return rc;
+}

@@ -1,0 +1,51 @@
+// cdmt_internal.h -- host-side description of one execute, shared by the API and the launchers.
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+namespace cdmt {
+
+struct Geometry {
+    int nsub, nfft, noverlap, nchan, ndec, ndm, in_dtype, chirp_ref;
+    double bw_mhz;
+    // derived
+    int step, mbin, hdisc, vdec;  // N-O, M, h, Vd
+    int n1, n2;                   // four-step split nfft = n1 * n2 (n1 >= n2)
+    int tw_hi_bits;               // w_N^e = hi[e >> lo_bits] * lo[e & mask]
+    int lo_bits;
+};
+
+// Device pointers into the workspace (all 256-byte aligned).
+struct Workspace {
+    double *dm;         // [ndm]
+    double *fcen;       // [nsub]
+    float2 *tw_n1;      // pass twiddles of the length-n1 forward transform
+    float2 *tw_n2;      // ... length-n2
+    float2 *tw_m;       // pass twiddles of the length-M backward transform
+    float2 *tw4_lo;     // four-step twiddle tables
+    float2 *tw4_hi;
+    float2 *bufA;       // [chunk_units][2][nfft] after pass A
+    float2 *spec;       // [chunk_units][2][nfft] shifted spectra Xs
+    size_t total_bytes;
+};
+
+size_t workspace_layout(const Geometry &g, int chunk_units, char *base, Workspace *ws);
+
+// Launchers: return cudaError_t of the launch; *launches is incremented per kernel launched.
+cudaError_t launch_init_tables(const Geometry &g, const Workspace &ws, const double *h_dm,
+                               const double *h_fcen, cudaStream_t st, long long *launches);
+cudaError_t launch_forward(const Geometry &g, const Workspace &ws, const void *d_in,
+                           long long in_stride_pol, int unit0, int nunits, float2 *spec_out,
+                           cudaStream_t st, long long *launches);
+cudaError_t launch_fused(const Geometry &g, const Workspace &ws, const float2 *spec, int unit0,
+                         int nunits, float *d_out, long long out_stride_dm, int dm_tile,
+                         int accurate, cudaStream_t st, long long *launches);
+cudaError_t launch_unpack(const Geometry &g, const void *d_in, long long in_stride_pol,
+                          int nblock, float2 *d_blocks, cudaStream_t st, long long *launches);
+cudaError_t launch_fp32_peak(float *d_scratch, int nblocks, int inner, cudaStream_t st);
+
+bool forward_len_supported(int L);
+bool fused_len_supported(int M);
+
+}  // namespace cdmt

@@ -1,0 +1,532 @@
+// cdmt_kernels.cu -- the sm_100a kernels of the cdmt hot path and their launchers.
+//
+//  k_init_twiddles / k_upload   constant tables into the workspace head
+//  k_unpack                     Alg. 1 l.95 as a stand-alone stage
+//  k_fwd_pass<L, MODE, IN>      forward FFT of length nfft = n1*n2 as two passes of a four-step
+//                               decomposition; pass A reads the raw voltages (unpack fused into
+//                               its loads), pass B writes the swapped-halves spectrum (l.96-97)
+//  k_fused<M, ...>              l.99-103 for a tile of DM trials: chirp on the fly, length-M
+//                               backward FFT, unpad, detect, Stokes I, time integration, pack
+#include "cdmt_fft.cuh"
+#include "cdmt_internal.h"
+
+namespace cdmt {
+
+// ------------------------------------------------------------------------------------
+// constant tables
+// ------------------------------------------------------------------------------------
+struct DoubleChunk {
+    double v[256];
+};
+
+__global__ void k_upload(double *dst, DoubleChunk c, int n)
+{
+    int i = threadIdx.x;
+    if (i < n) dst[i] = c.v[i];
+}
+
+// pass twiddles of RadixPlan<L> (runtime evaluation of the same layout)
+__global__ void k_init_pass_twiddles(float2 *tw, int L, int sign)
+{
+    int log2L = 31 - __clz(L);
+    int n16 = log2L / 4, rest = 1 << (log2L % 4);
+    int npass = n16 + (rest > 1 ? 1 : 0);
+    int off = 0, ns = 1;
+    for (int p = 0; p < npass; ++p) {
+        int R = p < n16 ? 16 : rest;
+        if (p >= 1) {
+            int cnt = (R - 1) * ns;
+            for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < cnt; e += gridDim.x * blockDim.x) {
+                int r = e / ns + 1, k = e % ns;
+                double s, c;
+                sincospi(2.0 * (double)k * (double)r / ((double)ns * (double)R), &s, &c);
+                tw[off + e] = make_float2((float)c, (float)(sign * s));
+            }
+            off += cnt;
+        }
+        ns *= R;
+    }
+}
+
+// four-step twiddles: exp(-2 pi i e / N) = hi[e >> lo_bits] * lo[e & (2^lo_bits - 1)]
+__global__ void k_init_fourstep(float2 *lo, float2 *hi, int N, int lo_bits)
+{
+    int nlo = 1 << lo_bits, nhi = N >> lo_bits;
+    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < nlo + nhi; e += gridDim.x * blockDim.x) {
+        double s, c;
+        if (e < nlo) {
+            sincospi(-2.0 * (double)e / (double)N, &s, &c);
+            lo[e] = make_float2((float)c, (float)s);
+        } else {
+            int a = e - nlo;
+            sincospi(-2.0 * (double)a * (double)nlo / (double)N, &s, &c);
+            hi[a] = make_float2((float)c, (float)s);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------
+// input words -> complex float (Alg. 1 l.95 "unpack")
+// ------------------------------------------------------------------------------------
+template <int IN>
+__device__ __forceinline__ float2 load_sample(const void *base, size_t idx);
+template <>
+__device__ __forceinline__ float2 load_sample<0>(const void *base, size_t idx)
+{
+    return __ldg(reinterpret_cast<const float2 *>(base) + idx);
+}
+template <>
+__device__ __forceinline__ float2 load_sample<1>(const void *base, size_t idx)
+{
+    char2 q = __ldg(reinterpret_cast<const char2 *>(base) + idx);
+    return make_float2((float)q.x, (float)q.y);
+}
+
+// blocks[(b nsub + s)][p][n] = in[s][p][b step + n]; 4 samples per thread
+template <int IN>
+__global__ void __launch_bounds__(256) k_unpack(const void *__restrict__ in, long long in_stride_pol,
+                                                int nsub, int nfft, int step, float2 *__restrict__ blocks)
+{
+    const int row = blockIdx.x;  // (b nsub + s) * 2 + p
+    const int unit = row >> 1, p = row & 1, b = unit / nsub, s = unit % nsub;
+    const size_t src0 = (size_t)(2 * s + p) * (size_t)in_stride_pol + (size_t)b * step;
+    float2 *dst = blocks + (size_t)row * nfft;
+    const int n0 = (blockIdx.y * 256 + threadIdx.x) * 4;
+    if (n0 >= nfft) return;
+    if (IN == 0) {
+        const float4 *src = reinterpret_cast<const float4 *>(reinterpret_cast<const float2 *>(in) + src0 + n0);
+        float4 a = __ldg(src), c = __ldg(src + 1);   // step and in_stride_pol are even: 16-byte aligned
+        reinterpret_cast<float4 *>(dst + n0)[0] = a;
+        reinterpret_cast<float4 *>(dst + n0)[1] = c;
+    } else {
+        const char2 *src = reinterpret_cast<const char2 *>(in) + src0 + n0;
+        float2 v[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            char2 q = __ldg(src + i);
+            v[i] = make_float2((float)q.x, (float)q.y);
+        }
+        reinterpret_cast<float4 *>(dst + n0)[0] = make_float4(v[0].x, v[0].y, v[1].x, v[1].y);
+        reinterpret_cast<float4 *>(dst + n0)[1] = make_float4(v[2].x, v[2].y, v[3].x, v[3].y);
+    }
+}
+
+// ------------------------------------------------------------------------------------
+// forward FFT, one pass of the four-step decomposition.
+//   n = n1i*n2 + n2i,  k = k1 + n1*k2
+//   pass A (MODE 0): for each n2i: T[k1][n2i] = w_N^(n2i k1) * sum_n1i x[n1i n2 + n2i] w_n1^(n1i k1)
+//   pass B (MODE 1): for each k1 : U[k1 + n1 k2] = sum_n2i T[k1][n2i] w_n2^(n2i k2), stored at the
+//                    swapped-halves position (k + N/2) mod N
+// A CTA transforms a tile of 16 transforms of length L held in shared memory as [elem][16+1].
+// ------------------------------------------------------------------------------------
+constexpr int FWD_BATCH = 16;
+
+template <int L, int MODE, int IN>
+__global__ void __launch_bounds__(L) k_fwd_pass(const void *__restrict__ src_v, float2 *__restrict__ dst,
+                                                const float2 *__restrict__ tw, const float2 *__restrict__ tw_lo,
+                                                const float2 *__restrict__ tw_hi, int lo_bits, int nfft, int n1,
+                                                int n2, int nsub, int step, long long in_stride_pol, int unit0)
+{
+    constexpr int NT = L;
+    using Plan = RadixPlan<L>;
+    using Addr = SmemAddr<FWD_BATCH>;
+    using Last = Pass<L, Plan::npass - 1, -1, NT, FWD_BATCH>;
+    extern __shared__ float2 smem[];
+    const int tid = threadIdx.x;
+    const int tile = blockIdx.y;       // MODE 0: 16 consecutive n2i; MODE 1: 16 consecutive k1
+    const int row = blockIdx.x;        // local (unit, pol)
+    const int p = row & 1;
+    const size_t plane = (size_t)row * nfft;
+
+    if (MODE == 0) {
+        const int unit = unit0 + (row >> 1), b = unit / nsub, s = unit % nsub;
+        const size_t src0 = (size_t)(2 * s + p) * (size_t)in_stride_pol + (size_t)b * step + (size_t)tile * FWD_BATCH;
+#pragma unroll 4
+        for (int e = tid; e < L * FWD_BATCH; e += NT) {
+            const int n1i = e / FWD_BATCH, col = e % FWD_BATCH;
+            smem[Addr::at(n1i, col)] = load_sample<IN>(src_v, src0 + (size_t)n1i * n2 + col);
+        }
+    } else {
+        const float2 *src = reinterpret_cast<const float2 *>(src_v) + plane + (size_t)tile * FWD_BATCH * n2;
+#pragma unroll 4
+        for (int e = tid; e < L * FWD_BATCH; e += NT) {
+            const int rr = e / L, n2i = e % L;
+            smem[Addr::at(n2i, rr)] = __ldg(src + (size_t)rr * n2 + n2i);
+        }
+    }
+    __syncthreads();
+    float2 v[16];
+    fft_passes<L, 0, -1, NT, FWD_BATCH, false>(v, smem, tw, tid);
+
+    const int nmask = nfft - 1;
+#pragma unroll
+    for (int u = 0; u < Last::U; ++u) {
+        const int col = Last::batch_of(tid, u);
+#pragma unroll
+        for (int q = 0; q < Last::R; ++q) {
+            const int k = Last::out_elem(tid, u, q);
+            float2 val = v[u * Last::R + q];
+            if (MODE == 0) {
+                const int n2i = tile * FWD_BATCH + col;
+                const int e = (int)(((long long)n2i * k) & nmask);
+                const float2 w = cmul(__ldg(tw_hi + (e >> lo_bits)), __ldg(tw_lo + (e & ((1 << lo_bits) - 1))));
+                dst[plane + (size_t)k * n2 + n2i] = cmul(val, w);
+            } else {
+                const int k1 = tile * FWD_BATCH + col;
+                const int kk = k1 + n1 * k;
+                dst[plane + ((kk + (nfft >> 1)) & nmask)] = val;
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------
+// fused per-DM kernel (Alg. 1 l.99-103 + time integration), one CTA per (unit, channel).
+// ------------------------------------------------------------------------------------
+template <bool ACCURATE>
+__device__ __forceinline__ float2 unit_phasor(float frac_cycles)
+{
+    float s, c;
+    if (ACCURATE) {
+        sincospif(2.0f * frac_cycles, &s, &c);
+    } else {
+        const float x = frac_cycles * 6.283185307179586f;
+        s = __sinf(x);
+        c = __cosf(x);
+    }
+    return make_float2(c, s);
+}
+
+template <int M, bool FASTDEC, bool ACCURATE>
+__global__ void __launch_bounds__(M / 16) k_fused(const float2 *__restrict__ spec, const float2 *__restrict__ tw,
+                                                 const double *__restrict__ dmlist, const double *__restrict__ fcen,
+                                                 float *__restrict__ out, long long out_stride_dm, int unit0,
+                                                 int nsub, int nchan, int nfft, int hdisc, int ndec, int vdec,
+                                                 int ndm, int dm_tile, int chirp_ref, double bw_mhz, float scale)
+{
+    constexpr int NT = M / 16;
+    using Plan = RadixPlan<M>;
+    using Addr = SmemAddr<1>;
+    using First = Pass<M, 0, +1, NT, 1>;
+    using Last = Pass<M, Plan::npass - 1, +1, NT, 1>;
+    extern __shared__ float2 smem[];
+    float2 *X = smem;                 // [2][M] the channel's spectrum, both pols
+    float2 *ex = smem + 2 * M;        // exchange buffer, Addr::size(M)
+    const int tid = threadIdx.x;
+    const int c = blockIdx.x % nchan;
+    const int ulocal = blockIdx.x / nchan;
+    const int unit = unit0 + ulocal, b = unit / nsub, s = unit % nsub;
+
+    // channel spectrum -> shared memory (read from HBM once per DM tile)
+    {
+        const float4 *src0 = reinterpret_cast<const float4 *>(spec + ((size_t)ulocal * 2) * nfft + (size_t)c * M);
+        const float4 *src1 = reinterpret_cast<const float4 *>(spec + ((size_t)ulocal * 2 + 1) * nfft + (size_t)c * M);
+        float4 *d0 = reinterpret_cast<float4 *>(X), *d1 = reinterpret_cast<float4 *>(X + M);
+        for (int e = tid; e < M / 2; e += NT) {
+            d0[e] = __ldg(src0 + e);
+            d1[e] = __ldg(src1 + e);
+        }
+    }
+
+    // Eq. 1 per bin this thread feeds to pass 0: phase = DM * g, g in cycles per unit DM
+    double g[16];
+    {
+        const double fc = fcen[s];
+        const double df = bw_mhz / (double)nfft;
+        double f0;
+        if (chirp_ref == 0) f0 = fc + ((double)c + 0.5 - 0.5 * (double)nchan) * bw_mhz / (double)nchan;
+        else f0 = fc;
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            const int m = First::in_elem(tid, 0, r);
+            const double f = (chirp_ref == 0) ? (double)(m - M / 2) * df : (double)(c * M + m - nfft / 2) * df;
+            g[r] = f * f / (2.41e-10 * f0 * f0 * (f0 + f));
+        }
+    }
+    __syncthreads();
+
+    const int nchan_total = nsub * nchan;
+    const int ochan = nchan_total - 1 - (s * nchan + c);
+    const int d_begin = blockIdx.y * dm_tile;
+    const int d_end = min(ndm, d_begin + dm_tile);
+
+    for (int d = d_begin; d < d_end; ++d) {
+        const double dm = dmlist[d];
+        float2 H[16];
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            const double t = fma(dm, g[r], 6755399441055744.0);   // 1.5 * 2^52: round to nearest integer
+            const double n = t - 6755399441055744.0;
+            const float fr = (float)fma(dm, g[r], -n);            // in [-0.5, 0.5]
+            H[r] = unit_phasor<ACCURATE>(fr);
+        }
+        float acc[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) acc[i] = 0.f;
+
+#pragma unroll 1
+        for (int p = 0; p < 2; ++p) {
+            float2 v[16];
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v[r] = cmul(X[p * M + First::in_elem(tid, 0, r)], H[r]);
+            __syncthreads();  // the exchange buffer is free (previous transform / decimation done)
+            fft_passes<M, 0, +1, NT, 1, true>(v, ex, tw, tid);
+#pragma unroll
+            for (int i = 0; i < 16; ++i) acc[i] = fmaf(v[i].x, v[i].x, fmaf(v[i].y, v[i].y, acc[i]));
+        }
+
+        float *outd = out + (size_t)d * (size_t)out_stride_dm + (size_t)b * vdec * nchan_total + ochan;
+        if (FASTDEC) {
+            // ndec consecutive samples sit in ndec adjacent lanes
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+                float a = acc[i];
+                for (int o = ndec >> 1; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+                acc[i] = a;
+            }
+            if ((tid & (ndec - 1)) == 0) {
+#pragma unroll
+                for (int u = 0; u < Last::U; ++u)
+#pragma unroll
+                    for (int q = 0; q < Last::R; ++q) {
+                        const int t = Last::out_elem(tid, u, q);
+                        if (t >= hdisc && t < M - hdisc)
+                            outd[(size_t)((t - hdisc) / ndec) * nchan_total] = acc[u * Last::R + q] * scale;
+                    }
+            }
+        } else {
+            float *I = reinterpret_cast<float *>(ex);
+            __syncthreads();
+#pragma unroll
+            for (int u = 0; u < Last::U; ++u)
+#pragma unroll
+                for (int q = 0; q < Last::R; ++q) I[Last::out_elem(tid, u, q)] = acc[u * Last::R + q];
+            __syncthreads();
+            for (int qd = tid; qd < vdec; qd += NT) {
+                float a = 0.f;
+                for (int r = 0; r < ndec; ++r) a += I[hdisc + qd * ndec + r];
+                outd[(size_t)qd * nchan_total] = a * scale;
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------
+// FP32 FMA rate (roofline denominator)
+// ------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(1024) k_fp32_peak(float *out, int inner)
+{
+    float a[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) a[i] = (float)(threadIdx.x + i) * 1e-3f;
+    const float m = 0.9999f, c = 1e-4f;
+    for (int it = 0; it < inner; ++it) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k)
+#pragma unroll
+            for (int i = 0; i < 8; ++i) a[i] = fmaf(a[i], m, c);
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += a[i];
+    if (s == 12345.678f) out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+cudaError_t launch_fp32_peak(float *d_scratch, int nblocks, int inner, cudaStream_t st)
+{
+    k_fp32_peak<<<nblocks, 1024, 0, st>>>(d_scratch, inner);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------
+// launchers
+// ------------------------------------------------------------------------------------
+static inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+static int pass_tw_size(int L)
+{
+    int log2L = 0;
+    while ((1 << log2L) < L) ++log2L;
+    int n16 = log2L / 4, rest = 1 << (log2L % 4), npass = n16 + (rest > 1 ? 1 : 0);
+    int off = 0, ns = 1;
+    for (int p = 0; p < npass; ++p) {
+        int R = p < n16 ? 16 : rest;
+        if (p >= 1) off += (R - 1) * ns;
+        ns *= R;
+    }
+    return off > 0 ? off : 1;
+}
+
+size_t workspace_layout(const Geometry &g, int chunk_units, char *base, Workspace *ws)
+{
+    size_t off = 0;
+    auto take = [&](size_t bytes) {
+        char *p = base ? base + off : nullptr;
+        off += align256(bytes);
+        return p;
+    };
+    Workspace w;
+    w.dm = reinterpret_cast<double *>(take(sizeof(double) * (size_t)g.ndm));
+    w.fcen = reinterpret_cast<double *>(take(sizeof(double) * (size_t)g.nsub));
+    w.tw_n1 = reinterpret_cast<float2 *>(take(sizeof(float2) * (size_t)pass_tw_size(g.n1)));
+    w.tw_n2 = reinterpret_cast<float2 *>(take(sizeof(float2) * (size_t)pass_tw_size(g.n2)));
+    w.tw_m = reinterpret_cast<float2 *>(take(sizeof(float2) * (size_t)pass_tw_size(g.mbin)));
+    w.tw4_lo = reinterpret_cast<float2 *>(take(sizeof(float2) * ((size_t)1 << g.lo_bits)));
+    w.tw4_hi = reinterpret_cast<float2 *>(take(sizeof(float2) * ((size_t)g.nfft >> g.lo_bits)));
+    const size_t plane = sizeof(float2) * 2 * (size_t)g.nfft * (size_t)chunk_units;
+    w.bufA = reinterpret_cast<float2 *>(take(plane));
+    w.spec = reinterpret_cast<float2 *>(take(plane));
+    w.total_bytes = off;
+    if (ws) *ws = w;
+    return off;
+}
+
+cudaError_t launch_init_tables(const Geometry &g, const Workspace &ws, const double *h_dm,
+                               const double *h_fcen, cudaStream_t st, long long *launches)
+{
+    auto upload = [&](double *dst, const double *src, int n) {
+        for (int o = 0; o < n; o += 256) {
+            DoubleChunk c;
+            int cnt = n - o < 256 ? n - o : 256;
+            for (int i = 0; i < cnt; ++i) c.v[i] = src[o + i];
+            for (int i = cnt; i < 256; ++i) c.v[i] = 0.0;
+            k_upload<<<1, 256, 0, st>>>(dst + o, c, cnt);
+            ++*launches;
+        }
+    };
+    upload(ws.dm, h_dm, g.ndm);
+    upload(ws.fcen, h_fcen, g.nsub);
+    k_init_pass_twiddles<<<8, 256, 0, st>>>(ws.tw_n1, g.n1, -1);
+    k_init_pass_twiddles<<<8, 256, 0, st>>>(ws.tw_n2, g.n2, -1);
+    k_init_pass_twiddles<<<32, 256, 0, st>>>(ws.tw_m, g.mbin, +1);
+    k_init_fourstep<<<8, 256, 0, st>>>(ws.tw4_lo, ws.tw4_hi, g.nfft, g.lo_bits);
+    *launches += 4;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_unpack(const Geometry &g, const void *d_in, long long in_stride_pol, int nblock,
+                          float2 *d_blocks, cudaStream_t st, long long *launches)
+{
+    dim3 grid((unsigned)(nblock * g.nsub * 2), (unsigned)((g.nfft / 4 + 255) / 256));
+    if (g.in_dtype == 0)
+        k_unpack<0><<<grid, 256, 0, st>>>(d_in, in_stride_pol, g.nsub, g.nfft, g.step, d_blocks);
+    else
+        k_unpack<1><<<grid, 256, 0, st>>>(d_in, in_stride_pol, g.nsub, g.nfft, g.step, d_blocks);
+    ++*launches;
+    return cudaGetLastError();
+}
+
+template <int L>
+static cudaError_t launch_fwd_L(int mode, const Geometry &g, const Workspace &ws, const void *src, float2 *dst,
+                                long long in_stride_pol, int unit0, int nunits, cudaStream_t st)
+{
+    const size_t smem = sizeof(float2) * SmemAddr<FWD_BATCH>::size(L);
+    const float2 *tw = (mode == 0) ? ws.tw_n1 : ws.tw_n2;
+    dim3 grid((unsigned)(nunits * 2), (unsigned)((mode == 0 ? g.n2 : g.n1) / FWD_BATCH));
+    cudaError_t e;
+#define CDMT_FWD(MODE, IN)                                                                                         \
+    do {                                                                                                           \
+        e = cudaFuncSetAttribute(k_fwd_pass<L, MODE, IN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+        if (e != cudaSuccess) return e;                                                                            \
+        k_fwd_pass<L, MODE, IN><<<grid, L, smem, st>>>(src, dst, tw, ws.tw4_lo, ws.tw4_hi, g.lo_bits, g.nfft,      \
+                                                       g.n1, g.n2, g.nsub, g.step, in_stride_pol, unit0);         \
+    } while (0)
+    if (mode == 0) {
+        if (g.in_dtype == 0) CDMT_FWD(0, 0);
+        else CDMT_FWD(0, 1);
+    } else {
+        CDMT_FWD(1, 0);
+    }
+#undef CDMT_FWD
+    return cudaGetLastError();
+}
+
+static cudaError_t launch_fwd_any(int L, int mode, const Geometry &g, const Workspace &ws, const void *src,
+                                  float2 *dst, long long in_stride_pol, int unit0, int nunits, cudaStream_t st)
+{
+    switch (L) {
+    case 16: return launch_fwd_L<16>(mode, g, ws, src, dst, in_stride_pol, unit0, nunits, st);
+    case 32: return launch_fwd_L<32>(mode, g, ws, src, dst, in_stride_pol, unit0, nunits, st);
+    case 64: return launch_fwd_L<64>(mode, g, ws, src, dst, in_stride_pol, unit0, nunits, st);
+    case 128: return launch_fwd_L<128>(mode, g, ws, src, dst, in_stride_pol, unit0, nunits, st);
+    case 256: return launch_fwd_L<256>(mode, g, ws, src, dst, in_stride_pol, unit0, nunits, st);
+    case 512: return launch_fwd_L<512>(mode, g, ws, src, dst, in_stride_pol, unit0, nunits, st);
+    case 1024: return launch_fwd_L<1024>(mode, g, ws, src, dst, in_stride_pol, unit0, nunits, st);
+    default: return cudaErrorInvalidValue;
+    }
+}
+
+bool forward_len_supported(int L) { return L >= 16 && L <= 1024 && (L & (L - 1)) == 0; }
+bool fused_len_supported(int M) { return M >= 16 && M <= 8192 && (M & (M - 1)) == 0; }
+
+cudaError_t launch_forward(const Geometry &g, const Workspace &ws, const void *d_in, long long in_stride_pol,
+                           int unit0, int nunits, float2 *spec_out, cudaStream_t st, long long *launches)
+{
+    cudaError_t e = launch_fwd_any(g.n1, 0, g, ws, d_in, ws.bufA, in_stride_pol, unit0, nunits, st);
+    if (e != cudaSuccess) return e;
+    ++*launches;
+    e = launch_fwd_any(g.n2, 1, g, ws, ws.bufA, spec_out, 0, unit0, nunits, st);
+    if (e != cudaSuccess) return e;
+    ++*launches;
+    return cudaSuccess;
+}
+
+template <int M>
+static cudaError_t launch_fused_M(const Geometry &g, const Workspace &ws, const float2 *spec, int unit0, int nunits,
+                                  float *d_out, long long out_stride_dm, int dm_tile, int accurate, cudaStream_t st)
+{
+    constexpr int NT = M / 16;
+    const size_t smem = sizeof(float2) * (2 * (size_t)M + SmemAddr<1>::size(M));
+    const int D = g.ndec;
+    const bool fast = NT >= 32 && D <= 32 && (D & (D - 1)) == 0 && (g.hdisc % D) == 0;
+    if (dm_tile <= 0 || dm_tile > g.ndm) dm_tile = g.ndm;
+    dim3 grid((unsigned)(nunits * g.nchan), (unsigned)((g.ndm + dm_tile - 1) / dm_tile));
+    const float scale = (float)(1.0 / ((double)g.nfft * (double)M));
+    cudaError_t e;
+#define CDMT_FUSED(FAST, ACC)                                                                                        \
+    do {                                                                                                             \
+        e = cudaFuncSetAttribute(k_fused<M, FAST, ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);     \
+        if (e != cudaSuccess) return e;                                                                              \
+        k_fused<M, FAST, ACC><<<grid, NT, smem, st>>>(spec, ws.tw_m, ws.dm, ws.fcen, d_out, out_stride_dm, unit0,    \
+                                                      g.nsub, g.nchan, g.nfft, g.hdisc, g.ndec, g.vdec, g.ndm,       \
+                                                      dm_tile, g.chirp_ref, g.bw_mhz, scale);                        \
+    } while (0)
+    if (fast) {
+        if (accurate) CDMT_FUSED(true, true);
+        else CDMT_FUSED(true, false);
+    } else {
+        if (accurate) CDMT_FUSED(false, true);
+        else CDMT_FUSED(false, false);
+    }
+#undef CDMT_FUSED
+    return cudaGetLastError();
+}
+
+cudaError_t launch_fused(const Geometry &g, const Workspace &ws, const float2 *spec, int unit0, int nunits,
+                         float *d_out, long long out_stride_dm, int dm_tile, int accurate, cudaStream_t st,
+                         long long *launches)
+{
+    cudaError_t e;
+    switch (g.mbin) {
+#define CDMT_CASE(MM)                                                                                      \
+    case MM:                                                                                               \
+        e = launch_fused_M<MM>(g, ws, spec, unit0, nunits, d_out, out_stride_dm, dm_tile, accurate, st);   \
+        break;
+        CDMT_CASE(16)
+        CDMT_CASE(32)
+        CDMT_CASE(64)
+        CDMT_CASE(128)
+        CDMT_CASE(256)
+        CDMT_CASE(512)
+        CDMT_CASE(1024)
+        CDMT_CASE(2048)
+        CDMT_CASE(4096)
+        CDMT_CASE(8192)
+#undef CDMT_CASE
+    default: return cudaErrorInvalidValue;
+    }
+    if (e == cudaSuccess) ++*launches;
+    return e;
+}
+
+}  // namespace cdmt

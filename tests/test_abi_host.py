@@ -1,0 +1,177 @@
+"""Host-side checks of the C ABI (no GPU): the library loads, exports what include/cdmt.h
+declares, validates arguments with status codes, and its block bookkeeping matches the
+SURVEY.md section 8 table for the five configs."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_1607_00909_b200 import synth
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def cdmt():
+    from paper_1607_00909_b200 import build
+    build.build()
+    from paper_1607_00909_b200 import cdmt as m
+    return m
+
+
+def header_functions():
+    txt = open(os.path.join(ROOT, "include", "cdmt.h")).read()
+    txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
+    return sorted(set(re.findall(r"\b(cdmt_[a-z0-9_]+)\s*\(", txt)))
+
+
+def test_library_exports_every_declared_symbol(cdmt):
+    lib = ctypes.CDLL(cdmt.LIB_PATH)
+    names = header_functions()
+    assert len(names) >= 14
+    for n in names:
+        assert hasattr(lib, n), n
+    assert sorted(cdmt.EXPORTS) == names          # the binding covers the whole header
+    for n in names:
+        assert hasattr(cdmt, n), "python binding lacks %s" % n
+
+
+def test_no_torch_types_in_the_abi():
+    txt = open(os.path.join(ROOT, "include", "cdmt.h")).read()
+    assert "torch" not in txt and "at::" not in txt and "Tensor" not in txt
+
+
+# SURVEY.md section 8 table:            B    V(dec)  out samples/chan  channels
+TABLE = {"c1": (5, 96, 480, 8), "c2": (18, 896, 16128, 160), "c3": (42, 192, 8064, 4608),
+         "c4": (31, 128, 3968, 2048), "c5": (127, 512, 65024, 512)}
+
+
+@pytest.mark.parametrize("name", synth.CONFIG_NAMES)
+def test_query_matches_scope_table(cdmt, name):
+    cfg = synth.make_config(name)
+    plan = cdmt.cdmt_plan_create(**cfg.plan_kwargs())
+    q = cdmt.cdmt_plan_query(plan, cfg.nsamp)
+    B, Vd, nout, nch = TABLE[name]
+    assert q["nblock"] == B == cfg.nblock
+    assert cfg.nvalid_dec == Vd
+    assert q["nout_per_chan"] == nout
+    assert cfg.nsub * cfg.nchan == nch
+    assert q["out_bytes"] == cfg.ndm * nout * nch * 4
+    assert q["nsamp_consumed"] == (B - 1) * cfg.step + cfg.nfft <= cfg.nsamp
+    assert q["workspace_bytes"] > 0
+    assert cdmt.cdmt_min_overlap(plan) <= cfg.noverlap      # every config's overlap covers its sweep
+    if name in ("c2", "c3", "c4", "c5"):
+        ps = cdmt.cdmt_plan_create(**cfg.plan_kwargs(synth.REF_SUBBAND))
+        mo = cdmt.cdmt_min_overlap(ps)
+        # c4's overlap is just short of the whole-subband sweep at the top DMs
+        assert (mo <= cfg.noverlap) == (name != "c4")
+
+
+def test_chunk_option_changes_workspace_only(cdmt):
+    cfg = synth.make_config("c3")
+    plan = cdmt.cdmt_plan_create(**cfg.plan_kwargs())
+    w0 = cdmt.cdmt_plan_query(plan, cfg.nsamp)["workspace_bytes"]
+    cdmt.cdmt_plan_set_option(plan, cdmt.OPT_CHUNK_UNITS, 64)
+    q = cdmt.cdmt_plan_query(plan, cfg.nsamp)
+    assert q["workspace_bytes"] < w0
+    assert abs(q["workspace_bytes"] - 2 * 64 * 2 * cfg.nfft * 8) < 2 ** 20
+    assert q["nblock"] == 42
+
+
+def bad(cdmt, status, **over):
+    kw = dict(nsub=2, fcen_mhz=[150.0, 150.2], bw_mhz=synth.BW_MHZ, nfft=4096, noverlap=1024,
+              nchan=8, ndec=4, dm=[0.0, 1.0])
+    kw.update(over)
+    with pytest.raises(cdmt.CdmtError) as e:
+        cdmt.cdmt_plan_create(**kw)
+    assert e.value.status == status, over
+
+
+def test_plan_create_validation(cdmt):
+    S, A = cdmt.ERR_SIZE, cdmt.ERR_ARG
+    bad(cdmt, S, nfft=4095)                    # not a power of two
+    bad(cdmt, S, nfft=128)                     # below the supported range
+    bad(cdmt, S, nfft=2 ** 21)
+    bad(cdmt, S, nchan=3)
+    bad(cdmt, S, nchan=512)                    # M = 8 < 16
+    bad(cdmt, S, nfft=2 ** 16, nchan=4)        # M = 16384 > 8192
+    bad(cdmt, S, noverlap=4096)                # >= nfft
+    bad(cdmt, S, noverlap=-16)
+    bad(cdmt, S, noverlap=1000)                # % (2 nchan) != 0
+    bad(cdmt, S, ndec=0)
+    bad(cdmt, S, ndec=5)                       # (nfft - noverlap) % (nchan ndec) != 0
+    bad(cdmt, A, bw_mhz=0.0)
+    bad(cdmt, A, bw_mhz=float("nan"))
+    bad(cdmt, A, fcen_mhz=[0.05, 150.0])       # fcen - bw/2 <= 0
+    bad(cdmt, A, dm=[0.0, float("inf")])
+    bad(cdmt, A, in_dtype=7)
+    bad(cdmt, A, chirp_ref=2)
+    lib = ctypes.CDLL(cdmt.LIB_PATH)
+    h = ctypes.c_void_p()
+    assert lib.cdmt_plan_create(ctypes.byref(h), 0, None, ctypes.c_double(0.2), 4096, 1024, 8, 4, 0, None, 0, 0) == A
+    assert h.value is None
+    assert lib.cdmt_plan_create(None, 1, None, ctypes.c_double(0.2), 4096, 1024, 8, 4, 1, None, 0, 0) == A
+    assert lib.cdmt_plan_destroy(None) == A
+
+
+def test_negative_dm_and_odd_ndec_are_legal(cdmt):
+    p = cdmt.cdmt_plan_create(1, [150.0], synth.BW_MHZ, 4096, 1024, 8, 3, [-5.0, 5.0])
+    assert cdmt.cdmt_plan_query(p, 4096)["nblock"] == 1
+    with pytest.raises(cdmt.CdmtError) as e:
+        cdmt.cdmt_plan_query(p, 4095)
+    assert e.value.status == cdmt.ERR_SIZE
+    with pytest.raises(cdmt.CdmtError):
+        cdmt.cdmt_plan_set_option(p, 99, 1)
+    with pytest.raises(cdmt.CdmtError):
+        cdmt.cdmt_plan_set_option(p, cdmt.OPT_PROFILE, 2)
+    cdmt.cdmt_plan_destroy(p)
+
+
+def test_execute_rejects_null_pointers_before_touching_cuda(cdmt):
+    """Argument validation happens on the host: these calls must return codes on a box with no GPU."""
+    p = cdmt.cdmt_plan_create(1, [150.0], synth.BW_MHZ, 4096, 1024, 8, 4, [0.0])
+    for args in [(0, 16384, 16384, 256, 10 ** 9, 256, 10 ** 9),
+                 (256, 16384, 16384, 0, 10 ** 9, 256, 10 ** 9),
+                 (256, 16384, 16384, 256, 10 ** 9, 0, 10 ** 9),
+                 (264, 16384, 16384, 256, 10 ** 9, 256, 10 ** 9)]:      # misaligned input
+        with pytest.raises(cdmt.CdmtError) as e:
+            cdmt.cdmt_execute(p, args[0], args[1], args[2], args[3], args[4], args[5], args[6], stream=0)
+        assert e.value.status == cdmt.ERR_ARG
+    with pytest.raises(cdmt.CdmtError) as e:
+        cdmt.cdmt_execute(p, 256, 16384, 8192, 256, 10 ** 9, 256, 10 ** 9, stream=0)     # stride < nsamp
+    assert e.value.status == cdmt.ERR_SIZE
+    with pytest.raises(cdmt.CdmtError) as e:
+        cdmt.cdmt_execute(p, 256, 16384, 16384, 256, 10, 256, 10 ** 9, stream=0)         # planes overlap
+    assert e.value.status == cdmt.ERR_SIZE
+
+
+def test_sweep_seconds_eq2_against_paper_values(cdmt):
+    vals = {}
+    for line in open(os.path.join(ROOT, "tests", "golden", "paper_values.txt")):
+        line = line.split("#", 1)[0].strip()
+        if line:
+            k, v = line.split("=")
+            vals[k.strip()] = float(v)
+    cw = synth.BW_MHZ / 8
+    assert abs(cdmt.cdmt_sweep_seconds(135.0, cw, vals["dm_J1810"]) * 1e3 - vals["td_ms_J1810"]) < 0.05
+    assert abs(cdmt.cdmt_sweep_seconds(135.0, cw, vals["dm_J2215"]) * 1e3 - vals["td_ms_J2215"]) < 0.05
+    assert cdmt.cdmt_strerror(0) == "ok" and "workspace" in cdmt.cdmt_strerror(3)
+    assert "sm_100a" in cdmt.cdmt_version()
+
+
+def test_product_path_does_not_import_the_oracle():
+    """The CUDA package must never route through oracle/ (and the oracle never imports the package)."""
+    pk = os.path.join(ROOT, "paper_1607_00909_b200")
+    for dirpath, _, files in os.walk(pk):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle", txt, flags=re.M), f
+                assert "cdmt_oracle" not in txt and "liboracle" not in txt, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            txt = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_1607_00909_b200" not in txt and "from paper_1607_00909_b200" not in txt
+            assert "libcdmt" not in txt

@@ -1,0 +1,230 @@
+"""GPU parity: the CUDA path through the C ABI against the CPU oracle, same seeded inputs.
+
+Tolerance (BASELINE.json north_star): max |delta| <= 1e-3 * rms of the oracle's filterbank,
+per DM trial; identical peak positions on injected pulses.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from oracle import cdmt_oracle as orc            # noqa: E402
+from paper_1607_00909_b200 import synth          # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def cdmt():
+    from paper_1607_00909_b200 import cdmt as m
+    assert torch.cuda.is_available()
+    return m
+
+
+TOL = 1e-3
+
+
+def check_filterbank(got, ref, tol=TOL):
+    assert got.shape == ref.shape
+    worst = 0.0
+    for d in range(ref.shape[0]):
+        rms = float(np.sqrt(np.mean(ref[d].astype(np.float64) ** 2)))
+        err = float(np.abs(got[d].astype(np.float64) - ref[d]).max())
+        assert err <= tol * rms, "DM %d: max|d| = %g, rms = %g" % (d, err, rms)
+        worst = max(worst, err / rms)
+    return worst
+
+
+def gpu_run(cdmt, cfg, x, chirp_ref=synth.REF_CHANNEL, opts=None):
+    plan = cdmt.cdmt_plan_create(**cfg.plan_kwargs(chirp_ref))
+    for k, v in (opts or {}).items():
+        cdmt.cdmt_plan_set_option(plan, k, v)
+    d_in = torch.from_numpy(x).cuda()
+    out = cdmt.run_on_device(plan, d_in, x.shape[2])
+    torch.cuda.synchronize()
+    return out.cpu().numpy(), plan
+
+
+# ---------------------------------------------------------------- stage a1: unpack / segment
+@pytest.mark.parametrize("in_dtype", [synth.IN_CF32, synth.IN_CI8])
+def test_unpack_blocks(cdmt, in_dtype):
+    cfg = synth.small_config(nsub=3, nsamp=4096 + 300, nfft=1024, noverlap=256, in_dtype=in_dtype)
+    x = synth.generate(cfg)
+    plan = cdmt.cdmt_plan_create(**cfg.plan_kwargs())
+    d_in = torch.from_numpy(x).cuda()
+    B = cfg.nblock
+    blocks = torch.zeros((B * cfg.nsub, 2, cfg.nfft), dtype=torch.complex64, device="cuda")
+    cdmt.cdmt_unpack(plan, d_in, cfg.nsamp, cfg.nsamp, blocks)
+    torch.cuda.synchronize()
+    got = blocks.cpu().numpy()
+    xc = x if in_dtype == synth.IN_CF32 else (x[..., 0].astype(np.float32) + 1j * x[..., 1].astype(np.float32))
+    for b in range(B):
+        for s in range(cfg.nsub):
+            exp = xc[s, :, b * cfg.step:b * cfg.step + cfg.nfft]
+            assert np.array_equal(got[b * cfg.nsub + s], exp.astype(np.complex64))   # bit exact
+
+
+# ---------------------------------------------------------------- stage a2-a3: forward FFT + swap
+@pytest.mark.parametrize("nfft", [256, 512, 1024, 4096, 8192, 65536, 131072, 262144])
+def test_forward_spectrum(cdmt, nfft):
+    nchan = 16 if nfft // 16 <= 8192 else nfft // 8192
+    cfg = synth.small_config(nsub=2, nsamp=nfft + (nfft // 2) * 2, nfft=nfft, noverlap=nfft // 2,
+                             nchan=nchan, ndec=1, dm=(0.0,))
+    x = synth.generate(cfg)
+    plan = cdmt.cdmt_plan_create(**cfg.plan_kwargs())
+    q = cdmt.cdmt_plan_query(plan, cfg.nsamp)
+    B = q["nblock"]
+    assert B == 3
+    d_in = torch.from_numpy(x).cuda()
+    spec = torch.zeros((B * cfg.nsub, 2, nfft), dtype=torch.complex64, device="cuda")
+    ws = torch.empty(q["workspace_bytes"], dtype=torch.uint8, device="cuda")
+    cdmt.cdmt_forward_spectrum(plan, d_in, cfg.nsamp, cfg.nsamp, spec, ws, ws.numel())
+    torch.cuda.synchronize()
+    got = spec.cpu().numpy()
+    p = orc.Params(**cfg.plan_kwargs())
+    for (b, s, pol) in [(0, 0, 0), (1, 1, 1), (2, 0, 1)]:
+        ref = orc.block_spectrum(p, x[s, pol], first=b * cfg.step)
+        err = np.abs(got[b * cfg.nsub + s, pol] - ref).max()
+        rms = np.sqrt(np.mean(np.abs(ref) ** 2))
+        assert err <= 2e-6 * rms * np.log2(nfft), (nfft, err / rms)
+
+
+# ---------------------------------------------------------------- whole path, small shapes
+SMALL = [
+    # nsub nsamp  nfft noverlap nchan ndec  (M)          comment
+    (1, 2 ** 14, 4096, 1024, 8, 4),         # c1 geometry (M=512)
+    (2, 4096 + 78, 1024, 256, 4, 2),        # M=256, ragged tail
+    (3, 3 * 768 + 256, 1024, 256, 64, 1),   # M=16: one thread per transform
+    (2, 2048, 1024, 0, 32, 4),              # M=32, no overlap
+    (1, 8192, 2048, 512, 32, 3),            # M=64, ndec=3 (general decimation path); step=1536=32*3*16
+    (2, 8192, 2048, 1024, 16, 8),           # M=128
+    (1, 2 ** 15, 8192, 2048, 8, 16),        # M=1024
+    (1, 2 ** 16, 16384, 4096, 8, 6),        # M=2048, ndec=6: step 12288 = 8*6*256
+    (2, 2 ** 17, 65536, 16384, 16, 16),     # c3 geometry (M=4096)
+    (1, 2 ** 17, 65536, 8192, 8, 8),        # c2 geometry (M=8192)
+    (1, 2 ** 16, 32768, 2048, 4, 64),       # M=8192, ndec=64 > warp
+    (1, 2 ** 13, 4096, 1024 + 16, 8, 1),    # h = 65: h % ndec irrelevant at ndec=1
+    (1, 2 ** 13, 4096, 1024 + 32, 8, 2),    # h = 66, ndec = 2 ok; step 3040 = 8*2*190
+    (1, 2 ** 13, 4096, 992, 8, 4),          # h = 62 -> h % ndec != 0 (general decimation path)
+]
+
+
+@pytest.mark.parametrize("shape", SMALL)
+@pytest.mark.parametrize("ref", [synth.REF_CHANNEL, synth.REF_SUBBAND])
+def test_small_shapes_full_parity(cdmt, shape, ref):
+    nsub, nsamp, nfft, noverlap, nchan, ndec = shape
+    if (nfft - noverlap) % (nchan * ndec) or noverlap % (2 * nchan):
+        pytest.skip("shape violates the divisibility rules")
+    cfg = synth.small_config(nsub=nsub, nsamp=nsamp, nfft=nfft, noverlap=noverlap, nchan=nchan,
+                             ndec=ndec, dm=(0.0, 2.0, -3.5, 41.25), f_lo=121.0)
+    x = synth.generate(cfg, chirp_ref=ref)
+    got, _ = gpu_run(cdmt, cfg, x, ref)
+    want = orc.run(orc.Params(**cfg.plan_kwargs(ref)), x)
+    check_filterbank(got, want)
+
+
+def test_c1_tiny_config(cdmt):
+    cfg = synth.make_config("c1")
+    for ref in (synth.REF_CHANNEL, synth.REF_SUBBAND):
+        x = synth.generate(cfg, chirp_ref=ref)
+        got, plan = gpu_run(cdmt, cfg, x, ref)
+        want = orc.run(orc.Params(**cfg.plan_kwargs(ref)), x)
+        check_filterbank(got, want)
+        # peak of the injected pulse: same DM trial, same sample
+        gi = np.unravel_index(got.sum(-1).argmax(), got.shape[:2])
+        wi = np.unravel_index(want.sum(-1).argmax(), want.shape[:2])
+        assert gi == wi
+        assert cfg.dm[gi[0]] == 4.0
+        assert cdmt.cdmt_last_launch_count(plan) >= 3
+
+
+def test_int8_input(cdmt):
+    cfg = synth.small_config(nsub=2, nsamp=2 ** 15, nfft=8192, noverlap=4096, nchan=8, ndec=8,
+                             dm=(0.0, 10.0, 99.9), in_dtype=synth.IN_CI8, f_lo=140.0)
+    x = synth.generate(cfg)
+    got, _ = gpu_run(cdmt, cfg, x)
+    want = orc.run(orc.Params(**cfg.plan_kwargs()), x)
+    check_filterbank(got, want)
+
+
+def test_options_do_not_change_results(cdmt):
+    cfg = synth.small_config(nsub=3, nsamp=2 ** 14, nfft=2048, noverlap=512, nchan=4, ndec=4,
+                             dm=tuple(np.arange(7) * 1.5))
+    x = synth.generate(cfg)
+    base, _ = gpu_run(cdmt, cfg, x)
+    want = orc.run(orc.Params(**cfg.plan_kwargs()), x)
+    check_filterbank(base, want)
+    for opts in ({cdmt.OPT_CHUNK_UNITS: 1}, {cdmt.OPT_CHUNK_UNITS: 5}, {cdmt.OPT_DM_TILE: 1},
+                 {cdmt.OPT_DM_TILE: 3}, {cdmt.OPT_CHUNK_UNITS: 4, cdmt.OPT_DM_TILE: 2}):
+        got, _ = gpu_run(cdmt, cfg, x, opts=opts)
+        assert np.array_equal(got, base), opts
+    acc, _ = gpu_run(cdmt, cfg, x, opts={cdmt.OPT_ACCURATE_SINCOS: 1})
+    check_filterbank(acc, want)
+
+
+def test_strided_input_and_output(cdmt):
+    """in_stride_pol > nsamp and out_stride_dm > plane size; streaming in two calls equals one call."""
+    cfg = synth.small_config(nsub=2, nsamp=8 * 768 + 256, nfft=1024, noverlap=256, nchan=4, ndec=2,
+                             dm=(0.0, 5.0, 9.0))
+    x = synth.generate(cfg)
+    want = orc.run(orc.Params(**cfg.plan_kwargs()), x)
+    plan = cdmt.cdmt_plan_create(**cfg.plan_kwargs())
+    d_in = torch.from_numpy(x).cuda()
+    T, step = cfg.nsamp, cfg.step
+    nch = cfg.nsub * cfg.nchan
+    B, Vd = cfg.nblock, cfg.nvalid_dec
+    out = torch.full((cfg.ndm, B * Vd + 5, nch), -1.0, dtype=torch.float32, device="cuda")
+    stride_dm = (B * Vd + 5) * nch
+    nb1 = 3
+    ns1 = (nb1 - 1) * step + cfg.nfft
+    q1 = cdmt.cdmt_plan_query(plan, ns1)
+    ws = torch.empty(cdmt.cdmt_plan_query(plan, T)["workspace_bytes"], dtype=torch.uint8, device="cuda")
+    assert q1["nblock"] == nb1
+    cdmt.cdmt_execute(plan, d_in, ns1, T, out, stride_dm, ws, ws.numel())
+    # second call: advance by nb1*step samples; output rows continue at nb1*Vd
+    off = nb1 * step
+    d_in2 = d_in.view(torch.float32).view(cfg.nsub, 2, T, 2)[:, :, off:, :]
+    out2 = out[:, nb1 * Vd:, :]
+    cdmt.cdmt_execute(plan, d_in2.data_ptr(), T - off, T, out2.data_ptr(), stride_dm, ws, ws.numel())
+    torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    check_filterbank(got[:, :B * Vd, :], want)
+    assert (got[:, B * Vd:, :] == -1.0).all()        # padding rows untouched
+
+
+def test_host_path_matches_device_path(cdmt):
+    cfg = synth.small_config(nsub=2, nsamp=2 ** 15, nfft=4096, noverlap=1024, nchan=8, ndec=4,
+                             dm=(0.0, 3.0, 6.0))
+    x = synth.generate(cfg)
+    dev, plan = gpu_run(cdmt, cfg, x)
+    h_in = torch.from_numpy(x).pin_memory()
+    h_out = torch.empty(dev.shape, dtype=torch.float32).pin_memory()
+    nbytes = cdmt.cdmt_host_scratch_bytes(plan, cfg.nsamp)
+    scratch = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    cdmt.cdmt_execute_host(plan, h_in.data_ptr(), cfg.nsamp, cfg.nsamp, h_out.data_ptr(), scratch, nbytes)
+    assert np.array_equal(h_out.numpy(), dev)
+
+
+def test_errors_are_codes_not_crashes(cdmt):
+    cfg = synth.small_config()
+    plan = cdmt.cdmt_plan_create(**cfg.plan_kwargs())
+    x = torch.zeros((cfg.nsub, 2, cfg.nsamp), dtype=torch.complex64, device="cuda")
+    q = cdmt.cdmt_plan_query(plan, cfg.nsamp)
+    out = torch.zeros((cfg.ndm, q["nout_per_chan"], cfg.nsub * cfg.nchan), device="cuda")
+    ws = torch.empty(q["workspace_bytes"], dtype=torch.uint8, device="cuda")
+    with pytest.raises(cdmt.CdmtError) as e:
+        cdmt.cdmt_execute(plan, x, cfg.nsamp, cfg.nsamp, out, out[0].numel(), ws, ws.numel() - 1024)
+    assert e.value.status == cdmt.ERR_WORKSPACE
+    with pytest.raises(cdmt.CdmtError) as e:
+        cdmt.cdmt_execute(plan, x, cfg.nfft - 1, cfg.nsamp, out, out[0].numel(), ws, ws.numel())
+    assert e.value.status == cdmt.ERR_SIZE
+    with pytest.raises(cdmt.CdmtError) as e:
+        cdmt.cdmt_execute(plan, x.data_ptr() + 8, cfg.nsamp, cfg.nsamp, out, out[0].numel(), ws, ws.numel())
+    assert e.value.status == cdmt.ERR_ARG
+    with pytest.raises(cdmt.CdmtError) as e:
+        cdmt.cdmt_execute(plan, x, cfg.nsamp, cfg.nsamp, out, out[0].numel() - 1, ws, ws.numel())
+    assert e.value.status == cdmt.ERR_SIZE
+    # and the plan still works afterwards
+    cdmt.cdmt_execute(plan, x, cfg.nsamp, cfg.nsamp, out, out[0].numel(), ws, ws.numel())
+    torch.cuda.synchronize()
+    assert float(out.abs().max()) == 0.0
