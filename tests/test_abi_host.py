@@ -173,5 +173,5 @@ def test_product_path_does_not_import_the_oracle():
     for f in os.listdir(os.path.join(ROOT, "oracle")):
         if f.endswith((".py", ".c")):
             txt = open(os.path.join(ROOT, "oracle", f)).read()
-            assert "import paper_1607_00909_b200" not in txt and "from paper_1607_00909_b200" not in txt
-            assert "libcdmt" not in txt
+            assert not re.search(r"^\s*(from|import)\s+paper_1607_00909_b200", txt, flags=re.M), f
+            assert "libcdmt" not in txt and "csrc" not in txt.replace("paper_1607_00909_b200/csrc/", ""), f
