@@ -58,7 +58,8 @@ enum {
     CDMT_OPT_CHUNK_UNITS = 0, /* (subband, block) units whose spectra are resident at once */
     CDMT_OPT_DM_TILE = 1,     /* DM trials looped inside one CTA of the fused kernel (0 = all) */
     CDMT_OPT_ACCURATE_SINCOS = 2, /* 1: sincospif instead of the fast approximation */
-    CDMT_OPT_PROFILE = 3      /* 1: record CUDA events round each kernel class (cdmt_profile_read) */
+    CDMT_OPT_PROFILE = 3,     /* 1: record CUDA events round each kernel class (cdmt_profile_read) */
+    CDMT_OPT_FORCE_GENERIC = 4 /* 1: always use the general fused kernel (any ndec / overlap) */
 };
 
 /*

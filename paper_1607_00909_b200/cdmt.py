@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libcdmt.so")
 OK, ERR_ARG, ERR_SIZE, ERR_WORKSPACE, ERR_CUDA, ERR_ALLOC = range(6)
 IN_CF32, IN_CI8 = 0, 1
 REF_CHANNEL, REF_SUBBAND = 0, 1
-OPT_CHUNK_UNITS, OPT_DM_TILE, OPT_ACCURATE_SINCOS, OPT_PROFILE = 0, 1, 2, 3
+OPT_CHUNK_UNITS, OPT_DM_TILE, OPT_ACCURATE_SINCOS, OPT_PROFILE, OPT_FORCE_GENERIC = 0, 1, 2, 3, 4
 
 EXPORTS = [
     "cdmt_plan_create", "cdmt_plan_destroy", "cdmt_plan_set_option", "cdmt_plan_query",

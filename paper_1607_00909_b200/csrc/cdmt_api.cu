@@ -18,6 +18,7 @@ struct cdmt_plan {
     int dm_tile;             // 0 = all
     int accurate;
     int profile;             // record CUDA events around each kernel class
+    int force_generic;       // use k_fused_generic even where the fast kernel applies
     long long last_launches;
     std::vector<cudaEvent_t> ev_pool;   // created lazily, reused
     size_t ev_used;
@@ -118,6 +119,7 @@ extern "C" int cdmt_plan_create(cdmt_plan **plan, int nsub, const double *fcen_m
     p->dm_tile = 0;
     p->accurate = 0;
     p->profile = 0;
+    p->force_generic = 0;
     p->ev_used = 0;
     p->last_launches = 0;
     *plan = p;
@@ -151,6 +153,10 @@ extern "C" int cdmt_plan_set_option(cdmt_plan *plan, int key, long long value)
     case CDMT_OPT_PROFILE:
         if (value != 0 && value != 1) return CDMT_ERR_ARG;
         plan->profile = (int)value;
+        return CDMT_OK;
+    case CDMT_OPT_FORCE_GENERIC:
+        if (value != 0 && value != 1) return CDMT_ERR_ARG;
+        plan->force_generic = (int)value;
         return CDMT_OK;
     default: return CDMT_ERR_ARG;
     }
@@ -246,7 +252,8 @@ static int run_chunks(cdmt_plan *plan, const void *d_in, long long in_stride_pol
         if (plan->profile) plan->spans.push_back({a, b, 0});
         if (d_out) {
             rc = check_cuda(launch_fused(g, ws, spec, (int)u0, n, d_out, out_stride_dm, plan->dm_tile,
-                                         plan->accurate, st, &plan->last_launches));
+                                         plan->accurate, plan->force_generic, plan->dm.data(),
+                                         plan->fcen.data(), st, &plan->last_launches));
             if (rc) return rc;
             if (!mark(&c)) return check_cuda(cudaErrorUnknown);
             if (plan->profile) plan->spans.push_back({b, c, 1});

@@ -1,0 +1,454 @@
+// cdmt_fused.cu -- the fused per-DM kernels (Alg. 1 l.99-103 + time integration):
+// one CTA per (subband, block, channel); the channel's spectrum of both polarisations stays
+// in shared memory while the CTA loops over a tile of DM trials, so the spectrum is read from
+// HBM once per DM tile and only the integrated float32 filterbank is written.
+//
+// Per DM trial and polarisation:  Z[m] = X[m] * exp(2 pi i DM g[m])      (Eq. 1)
+//                                 y[t] = sum_m Z[m] exp(+2 pi i m t / M)
+//   (the per-channel swap of halves only multiplies y[t] by (-1)^t, which detection removes)
+// then |y_0|^2 + |y_1|^2, unpad, sum over ndec samples, scale 1/(N M), pack.
+//
+//  k_fused_fast<M, LOGD>   ndec = 2^LOGD <= 32, h % ndec == 0, M >= 512: chirp phase from a
+//                          per-thread degree-5 polynomial in fp64, in-place radix-16 passes
+//                          (3 barriers per transform), warp-shuffle reduce-scatter for the time
+//                          integration; <= 128 registers so that two CTAs share an SM at M = 4096.
+//  k_fused_generic<M>      any ndec / overlap / M >= 16: exact per-bin phase constants in
+//                          registers, autosort passes, integration through shared memory.
+#include "cdmt_fft.cuh"
+#include "cdmt_internal.h"
+
+namespace cdmt {
+
+template <bool ACCURATE>
+__device__ __forceinline__ float2 unit_phasor(float frac_cycles)
+{
+    float s, c;
+    if (ACCURATE) {
+        sincospif(2.0f * frac_cycles, &s, &c);
+    } else {
+        const float x = frac_cycles * 6.283185307179586f;
+        s = __sinf(x);
+        c = __cosf(x);
+    }
+    return make_float2(c, s);
+}
+
+__device__ __forceinline__ float2 unit_phasor_rt(float frac_cycles, int accurate)
+{
+    return accurate ? unit_phasor<true>(frac_cycles) : unit_phasor<false>(frac_cycles);
+}
+
+// fractional part in [-0.5, 0.5] of dm * g, exact to fp64 rounding
+__device__ __forceinline__ float frac_cycles(double dm, double g)
+{
+    const double magic = 6755399441055744.0;  // 1.5 * 2^52: adding it rounds to the nearest integer
+    const double n = fma(dm, g, magic) - magic;
+    return (float)fma(dm, g, -n);
+}
+
+struct FusedArgs {
+    const float2 *spec;      // [units][2][nfft] swapped-halves spectra of this chunk
+    const float2 *tw;        // pass twiddles of the length-M backward transform
+    const double *dmlist;
+    const double *fcen;
+    float *out;
+    long long out_stride_dm;
+    int unit0, nsub, nchan, nfft, hdisc, ndec, vdec, ndm, dm_tile, chirp_ref, accurate;
+    double bw_mhz;
+    float scale;
+};
+
+// frequency set-up shared by both kernels: nu_0 of Eq. 1 and the offset of bin m (MHz)
+__device__ __forceinline__ void chirp_axes(const FusedArgs &a, int s, int c, int M, double *f0, double *f_bin0,
+                                           double *df)
+{
+    const double fc = a.fcen[s];
+    *df = a.bw_mhz / (double)a.nfft;
+    if (a.chirp_ref == 0) {
+        *f0 = fc + ((double)c + 0.5 - 0.5 * (double)a.nchan) * a.bw_mhz / (double)a.nchan;
+        *f_bin0 = -(double)(M / 2) * *df;
+    } else {
+        *f0 = fc;
+        *f_bin0 = (double)(c * M - a.nfft / 2) * *df;
+    }
+}
+
+// ------------------------------------------------------------------------------------
+// generic kernel
+// ------------------------------------------------------------------------------------
+template <int M>
+__global__ void __launch_bounds__(M / 16) k_fused_generic(const FusedArgs a)
+{
+    constexpr int NT = M / 16;
+    using Plan = RadixPlan<M>;
+    using First = Pass<M, 0, +1, NT, 1>;
+    using Last = Pass<M, Plan::npass - 1, +1, NT, 1>;
+    extern __shared__ float2 smem[];
+    float2 *X = smem;           // [2][M]
+    float2 *ex = smem + 2 * M;  // SmemAddr<1>::size(M)
+    const int tid = threadIdx.x;
+    const int c = blockIdx.x % a.nchan;
+    const int ulocal = blockIdx.x / a.nchan;
+    const int unit = a.unit0 + ulocal, b = unit / a.nsub, s = unit % a.nsub;
+    {
+        const float4 *src0 = reinterpret_cast<const float4 *>(a.spec + ((size_t)ulocal * 2) * a.nfft + (size_t)c * M);
+        const float4 *src1 = reinterpret_cast<const float4 *>(a.spec + ((size_t)ulocal * 2 + 1) * a.nfft + (size_t)c * M);
+        float4 *d0 = reinterpret_cast<float4 *>(X), *d1 = reinterpret_cast<float4 *>(X + M);
+        for (int e = tid; e < M / 2; e += NT) {
+            d0[e] = __ldg(src0 + e);
+            d1[e] = __ldg(src1 + e);
+        }
+    }
+    double g[16];  // Eq. 1 per bin: phase = DM * g, cycles
+    {
+        double f0, fb0, df;
+        chirp_axes(a, s, c, M, &f0, &fb0, &df);
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            const double f = fb0 + (double)First::in_elem(tid, 0, r) * df;
+            g[r] = f * f / (2.41e-10 * f0 * f0 * (f0 + f));
+        }
+    }
+    __syncthreads();
+    const int nchan_total = a.nsub * a.nchan;
+    const int ochan = nchan_total - 1 - (s * a.nchan + c);
+    const int d_begin = blockIdx.y * a.dm_tile;
+    const int d_end = min(a.ndm, d_begin + a.dm_tile);
+    for (int d = d_begin; d < d_end; ++d) {
+        const double dm = a.dmlist[d];
+        float2 H[16];
+#pragma unroll
+        for (int r = 0; r < 16; ++r) H[r] = unit_phasor_rt(frac_cycles(dm, g[r]), a.accurate);
+        float acc[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) acc[i] = 0.f;
+#pragma unroll 1
+        for (int p = 0; p < 2; ++p) {
+            float2 v[16];
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v[r] = cmul(X[p * M + First::in_elem(tid, 0, r)], H[r]);
+            __syncthreads();  // exchange buffer free
+            fft_passes<M, 0, +1, NT, 1, true>(v, ex, a.tw, tid);
+#pragma unroll
+            for (int i = 0; i < 16; ++i) acc[i] = fmaf(v[i].x, v[i].x, fmaf(v[i].y, v[i].y, acc[i]));
+        }
+        float *outd = a.out + (size_t)d * (size_t)a.out_stride_dm + (size_t)b * a.vdec * nchan_total + ochan;
+        float *I = reinterpret_cast<float *>(ex);
+        __syncthreads();
+#pragma unroll
+        for (int u = 0; u < Last::U; ++u)
+#pragma unroll
+            for (int q = 0; q < Last::R; ++q) I[Last::out_elem(tid, u, q)] = acc[u * Last::R + q];
+        __syncthreads();
+        for (int qd = tid; qd < a.vdec; qd += NT) {
+            float sum = 0.f;
+            for (int r = 0; r < a.ndec; ++r) sum += I[a.hdisc + qd * a.ndec + r];
+            outd[(size_t)qd * nchan_total] = sum * a.scale;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------
+// fast kernel: in-place passes.  Digits: pass p transforms input digit i_p (stride M/(R_0..R_p))
+// into output digit o_p (weight T_p = R_0..R_(p-1)).  A value with digits (d_0, d_1, ..)
+// lives at d_0 * (M/16 + 1) + sum_{q>=1} d_q A_q, A_q = product of the radices after q; the
+// odd pitch of d_0 makes every access of 16 consecutive d_0 bank-conflict free.
+// ------------------------------------------------------------------------------------
+template <int M>
+struct InplacePlan {
+    using Plan = RadixPlan<M>;
+    static constexpr int NT = M / 16;
+    static constexpr int A0 = M / 16 + 1;
+    static constexpr int size = 16 * A0;
+    static constexpr int after(int p)  // product of radices after pass p
+    {
+        int n = 1;
+        for (int q = p + 1; q < Plan::npass; ++q) n *= Plan::radix(q);
+        return n;
+    }
+};
+
+template <int M, int P>
+struct InplacePass {
+    using Plan = RadixPlan<M>;
+    using IP = InplacePlan<M>;
+    static constexpr int NT = IP::NT;
+    static constexpr int R = Plan::radix(P);
+    static constexpr int T = Plan::ns(P);     // weight of the output digit
+    static constexpr int A = IP::after(P);    // address stride of the digit
+    static constexpr int U = 16 / R;
+    static constexpr int TWOFF = Plan::tw_offset(P);
+    static constexpr int A1 = IP::after(1);
+    static constexpr int A2 = IP::after(2);
+
+    // shared-memory address of element x = 0 of butterfly beta
+    static __device__ __forceinline__ int base(int beta)
+    {
+        const int K = beta % T, lo = beta / T;
+        int addr = (K & 15) * IP::A0 + lo;
+        if (P >= 2) addr += ((K >> 4) & 15) * A1;
+        if (P >= 3) addr += ((K >> 8) & 15) * A2;
+        return addr;
+    }
+    static __device__ __forceinline__ void load(const float2 *ex, float2 *v, int tid)
+    {
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int bs = base(tid + u * NT);
+#pragma unroll
+            for (int x = 0; x < R; ++x) v[u * R + x] = ex[bs + x * A];
+        }
+    }
+    static __device__ __forceinline__ void store(float2 *ex, const float2 *v, int tid)
+    {
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int bs = base(tid + u * NT);
+#pragma unroll
+            for (int x = 0; x < R; ++x) ex[bs + x * A] = v[u * R + x];
+        }
+    }
+    static __device__ __forceinline__ void compute(float2 *v, const float2 *__restrict__ tw, int tid)
+    {
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int K = (tid + u * NT) % T;
+            const float2 *t = tw + TWOFF + K;
+#pragma unroll
+            for (int x = 1; x < R; ++x) v[u * R + x] = cmul(v[u * R + x], __ldg(t + (x - 1) * T));
+            Dft<R, +1>::run(v + u * R);
+        }
+    }
+};
+
+template <int M, int P>
+__device__ __forceinline__ void inplace_tail(float2 *v, float2 *ex, const float2 *__restrict__ tw, int tid)
+{
+    using Ps = InplacePass<M, P>;
+    __syncthreads();  // previous pass stored
+    Ps::load(ex, v, tid);
+    Ps::compute(v, tw, tid);
+    if constexpr (P + 1 < RadixPlan<M>::npass) {
+        Ps::store(ex, v, tid);  // same slots this thread just read
+        inplace_tail<M, P + 1>(v, ex, tw, tid);
+    }
+}
+
+// reduce-scatter over 2^LOGD adjacent lanes: in[n], n < 16, becomes out[j] = sum over the lane
+// group of slot n = (lane & (D-1)) + D j
+template <int LOGD, int S = 0>
+__device__ __forceinline__ void lane_reduce_scatter(float *a, int lane)
+{
+    if constexpr (S < LOGD) {
+        constexpr int cnt = 16 >> S;  // values held before this stage
+        const bool up = (lane >> S) & 1;
+#pragma unroll
+        for (int j = 0; j < cnt / 2; ++j) {
+            const float lo = a[2 * j], hi = a[2 * j + 1];
+            const float send = up ? lo : hi;
+            const float keep = up ? hi : lo;
+            a[j] = keep + __shfl_xor_sync(0xffffffffu, send, 1 << S);
+        }
+        lane_reduce_scatter<LOGD, S + 1>(a, lane);
+    }
+}
+
+template <int M, int LOGD>
+__global__ void __launch_bounds__(M / 16, (512 / (M / 16) > 16 ? 16 : (512 / (M / 16) < 1 ? 1 : 512 / (M / 16))))
+k_fused_fast(const FusedArgs a)
+{
+    constexpr int NT = M / 16;
+    constexpr int D = 1 << LOGD;
+    constexpr int LS = LOGD < 4 ? LOGD : 4;  // reduce-scatter stages (16 values per thread)
+    constexpr int NKEEP = 16 >> LS;          // integrated samples per thread per DM
+    using Plan = RadixPlan<M>;
+    using IP = InplacePlan<M>;
+    using LastP = InplacePass<M, Plan::npass - 1>;
+    static_assert(Plan::npass >= 2 && NT >= 32, "fast path needs M >= 512");
+    extern __shared__ float2 smem[];
+    float2 *X = smem;           // [2][M]
+    float2 *ex = smem + 2 * M;  // IP::size
+    const int tid = threadIdx.x;
+    const int lane = tid & 31;
+    const int c = blockIdx.x % a.nchan;
+    const int ulocal = blockIdx.x / a.nchan;
+    const int unit = a.unit0 + ulocal, b = unit / a.nsub, s = unit % a.nsub;
+    {
+        const float4 *src0 = reinterpret_cast<const float4 *>(a.spec + ((size_t)ulocal * 2) * a.nfft + (size_t)c * M);
+        const float4 *src1 = reinterpret_cast<const float4 *>(a.spec + ((size_t)ulocal * 2 + 1) * a.nfft + (size_t)c * M);
+        float4 *d0 = reinterpret_cast<float4 *>(X), *d1 = reinterpret_cast<float4 *>(X + M);
+#pragma unroll 4
+        for (int e = tid; e < M / 2; e += NT) {
+            d0[e] = __ldg(src0 + e);
+            d1[e] = __ldg(src1 + e);
+        }
+    }
+    // Eq. 1 along this thread's bins m_r = tid + r M/16: g(f_a + b r) = sum_k ck r^k (Taylor in
+    // b r / (f0 + f_a) <= 1e-3; the host checks that the r^6 term is below 1e-7 cycles)
+    double c0, c1, c2, c3, c4, c5;
+    {
+        double f0, fb0, df;
+        chirp_axes(a, s, c, M, &f0, &fb0, &df);
+        const double fa = fb0 + (double)tid * df, bb = (double)NT * df;
+        const double kc = 1.0 / (2.41e-10 * f0 * f0);
+        const double sa = f0 + fa, e = bb / sa, pp = kc * f0 * f0 / sa;
+        c0 = kc * fa * fa / sa;
+        c1 = kc * (fa * fa + 2.0 * fa * f0) / (sa * sa) * bb;
+        c2 = pp * e * e;
+        c3 = -c2 * e;
+        c4 = -c3 * e;
+        c5 = -c4 * e;
+    }
+    const int nchan_total = a.nsub * a.nchan;
+    const int ochan = nchan_total - 1 - (s * a.nchan + c);
+    float *out0 = a.out + (size_t)b * a.vdec * nchan_total + ochan;
+    const int d_begin = blockIdx.y * a.dm_tile;
+    const int d_end = min(a.ndm, d_begin + a.dm_tile);
+    __syncthreads();
+
+#pragma unroll 1
+    for (int d = d_begin; d < d_end; ++d) {
+        const double dm = a.dmlist[d];
+        // phase polynomial of this DM (scaling the coefficients keeps the evaluation inside the loop)
+        const double p0 = dm * c0, p1 = dm * c1, p2 = dm * c2, p3 = dm * c3, p4 = dm * c4, p5 = dm * c5;
+        float2 H[16];
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            const double rr = (double)r;
+            const double phi = fma(fma(fma(fma(fma(p5, rr, p4), rr, p3), rr, p2), rr, p1), rr, p0);
+            const double magic = 6755399441055744.0;
+            const double n = (phi + magic) - magic;
+            H[r] = unit_phasor<false>((float)(phi - n));
+        }
+        float res[NKEEP];
+#pragma unroll 1
+        for (int p = 0; p < 2; ++p) {
+            float2 v[16];
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v[r] = cmul(X[p * M + tid + r * NT], H[r]);
+            Dft<16, +1>::run(v);
+            __syncthreads();  // every thread has finished reading the previous transform
+#pragma unroll
+            for (int q = 0; q < 16; ++q) ex[q * IP::A0 + tid] = v[q];
+            inplace_tail<M, 1>(v, ex, a.tw, tid);
+            // v[u R + x] = y[t], t = tid + NT (u + U x): reorder to n = u + U x, detect
+            float pw[16];
+#pragma unroll
+            for (int u = 0; u < LastP::U; ++u)
+#pragma unroll
+                for (int x = 0; x < LastP::R; ++x) {
+                    const float2 y = v[u * LastP::R + x];
+                    pw[u + LastP::U * x] = fmaf(y.x, y.x, y.y * y.y);
+                }
+            lane_reduce_scatter<LS>(pw, lane);
+            if constexpr (LOGD > LS) pw[0] += __shfl_xor_sync(0xffffffffu, pw[0], 16);
+#pragma unroll
+            for (int j = 0; j < NKEEP; ++j) res[j] = (p == 0) ? pw[j] : res[j] + pw[j];
+        }
+        float *outd = out0 + (size_t)d * (size_t)a.out_stride_dm;
+#pragma unroll
+        for (int j = 0; j < NKEEP; ++j) {
+            const int n = (lane & ((1 << LS) - 1)) + (1 << LS) * j;
+            const int t0 = (tid & ~(D - 1)) + NT * n;  // first sample of the integrated group
+            if ((lane & (D - 1)) < (1 << LS) && t0 >= a.hdisc && t0 < M - a.hdisc)
+                outd[(size_t)((t0 - a.hdisc) >> LOGD) * nchan_total] = res[j] * a.scale;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------
+// launch
+// ------------------------------------------------------------------------------------
+template <int M>
+static cudaError_t launch_generic_M(const FusedArgs &fa, dim3 grid, cudaStream_t st)
+{
+    const size_t smem = sizeof(float2) * (2 * (size_t)M + SmemAddr<1>::size(M));
+    cudaError_t e = cudaFuncSetAttribute(k_fused_generic<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_fused_generic<M><<<grid, M / 16, smem, st>>>(fa);
+    return cudaGetLastError();
+}
+
+template <int M, int LOGD>
+static cudaError_t launch_fast_MD(const FusedArgs &fa, dim3 grid, cudaStream_t st)
+{
+    const size_t smem = sizeof(float2) * (2 * (size_t)M + InplacePlan<M>::size);
+    cudaError_t e = cudaFuncSetAttribute(k_fused_fast<M, LOGD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_fused_fast<M, LOGD><<<grid, M / 16, smem, st>>>(fa);
+    return cudaGetLastError();
+}
+
+template <int M>
+static cudaError_t launch_fast_M(int logd, const FusedArgs &fa, dim3 grid, cudaStream_t st)
+{
+    switch (logd) {
+    case 0: return launch_fast_MD<M, 0>(fa, grid, st);
+    case 1: return launch_fast_MD<M, 1>(fa, grid, st);
+    case 2: return launch_fast_MD<M, 2>(fa, grid, st);
+    case 3: return launch_fast_MD<M, 3>(fa, grid, st);
+    case 4: return launch_fast_MD<M, 4>(fa, grid, st);
+    case 5: return launch_fast_MD<M, 5>(fa, grid, st);
+    default: return cudaErrorInvalidValue;
+    }
+}
+
+// Can the degree-5 phase polynomial be used?  Bound on the first neglected term (cycles).
+static bool poly_phase_ok(const Geometry &g, const double *h_dm, const double *h_fcen)
+{
+    double dmax = 0.0, fmin = h_fcen[0];
+    for (int d = 0; d < g.ndm; ++d) dmax = fabs(h_dm[d]) > dmax ? fabs(h_dm[d]) : dmax;
+    for (int s = 0; s < g.nsub; ++s) fmin = h_fcen[s] < fmin ? h_fcen[s] : fmin;
+    const double flo = fmin - 0.5 * g.bw_mhz;
+    const double x = 15.0 * (g.mbin / 16) * (g.bw_mhz / g.nfft) / flo;
+    const double P = dmax / (2.41e-10 * flo);
+    return P * x * x * x * x * x * x < 1e-7;
+}
+
+cudaError_t launch_fused(const Geometry &g, const Workspace &ws, const float2 *spec, int unit0, int nunits,
+                         float *d_out, long long out_stride_dm, int dm_tile, int accurate, int force_generic,
+                         const double *h_dm, const double *h_fcen, cudaStream_t st, long long *launches)
+{
+    const int M = g.mbin, D = g.ndec;
+    if (dm_tile <= 0 || dm_tile > g.ndm) dm_tile = g.ndm;
+    dim3 grid((unsigned)(nunits * g.nchan), (unsigned)((g.ndm + dm_tile - 1) / dm_tile));
+    FusedArgs fa;
+    fa.spec = spec; fa.tw = ws.tw_m; fa.dmlist = ws.dm; fa.fcen = ws.fcen; fa.out = d_out;
+    fa.out_stride_dm = out_stride_dm; fa.unit0 = unit0; fa.nsub = g.nsub; fa.nchan = g.nchan; fa.nfft = g.nfft;
+    fa.hdisc = g.hdisc; fa.ndec = g.ndec; fa.vdec = g.vdec; fa.ndm = g.ndm; fa.dm_tile = dm_tile;
+    fa.chirp_ref = g.chirp_ref; fa.accurate = accurate; fa.bw_mhz = g.bw_mhz;
+    fa.scale = (float)(1.0 / ((double)g.nfft * (double)M));
+    int logd = 0;
+    while ((1 << logd) < D) ++logd;
+    const bool fast = !force_generic && !accurate && M >= 512 && D <= 32 && (1 << logd) == D && (g.hdisc % D) == 0 &&
+                      poly_phase_ok(g, h_dm, h_fcen);
+    cudaError_t e = cudaErrorInvalidValue;
+    if (fast) {
+        switch (M) {
+        case 512: e = launch_fast_M<512>(logd, fa, grid, st); break;
+        case 1024: e = launch_fast_M<1024>(logd, fa, grid, st); break;
+        case 2048: e = launch_fast_M<2048>(logd, fa, grid, st); break;
+        case 4096: e = launch_fast_M<4096>(logd, fa, grid, st); break;
+        case 8192: e = launch_fast_M<8192>(logd, fa, grid, st); break;
+        default: break;
+        }
+    } else {
+        switch (M) {
+        case 16: e = launch_generic_M<16>(fa, grid, st); break;
+        case 32: e = launch_generic_M<32>(fa, grid, st); break;
+        case 64: e = launch_generic_M<64>(fa, grid, st); break;
+        case 128: e = launch_generic_M<128>(fa, grid, st); break;
+        case 256: e = launch_generic_M<256>(fa, grid, st); break;
+        case 512: e = launch_generic_M<512>(fa, grid, st); break;
+        case 1024: e = launch_generic_M<1024>(fa, grid, st); break;
+        case 2048: e = launch_generic_M<2048>(fa, grid, st); break;
+        case 4096: e = launch_generic_M<4096>(fa, grid, st); break;
+        case 8192: e = launch_generic_M<8192>(fa, grid, st); break;
+        default: break;
+        }
+    }
+    if (e == cudaSuccess) ++*launches;
+    return e;
+}
+
+}  // namespace cdmt

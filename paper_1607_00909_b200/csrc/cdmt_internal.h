@@ -40,7 +40,8 @@ cudaError_t launch_forward(const Geometry &g, const Workspace &ws, const void *d
                            cudaStream_t st, long long *launches);
 cudaError_t launch_fused(const Geometry &g, const Workspace &ws, const float2 *spec, int unit0,
                          int nunits, float *d_out, long long out_stride_dm, int dm_tile,
-                         int accurate, cudaStream_t st, long long *launches);
+                         int accurate, int force_generic, const double *h_dm, const double *h_fcen,
+                         cudaStream_t st, long long *launches);
 cudaError_t launch_unpack(const Geometry &g, const void *d_in, long long in_stride_pol,
                           int nblock, float2 *d_blocks, cudaStream_t st, long long *launches);
 cudaError_t launch_fp32_peak(float *d_scratch, int nblocks, int inner, cudaStream_t st);

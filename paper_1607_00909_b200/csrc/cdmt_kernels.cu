@@ -181,137 +181,6 @@ __global__ void __launch_bounds__(L) k_fwd_pass(const void *__restrict__ src_v, 
 }
 
 // ------------------------------------------------------------------------------------
-// fused per-DM kernel (Alg. 1 l.99-103 + time integration), one CTA per (unit, channel).
-// ------------------------------------------------------------------------------------
-template <bool ACCURATE>
-__device__ __forceinline__ float2 unit_phasor(float frac_cycles)
-{
-    float s, c;
-    if (ACCURATE) {
-        sincospif(2.0f * frac_cycles, &s, &c);
-    } else {
-        const float x = frac_cycles * 6.283185307179586f;
-        s = __sinf(x);
-        c = __cosf(x);
-    }
-    return make_float2(c, s);
-}
-
-template <int M, bool FASTDEC, bool ACCURATE>
-__global__ void __launch_bounds__(M / 16) k_fused(const float2 *__restrict__ spec, const float2 *__restrict__ tw,
-                                                 const double *__restrict__ dmlist, const double *__restrict__ fcen,
-                                                 float *__restrict__ out, long long out_stride_dm, int unit0,
-                                                 int nsub, int nchan, int nfft, int hdisc, int ndec, int vdec,
-                                                 int ndm, int dm_tile, int chirp_ref, double bw_mhz, float scale)
-{
-    constexpr int NT = M / 16;
-    using Plan = RadixPlan<M>;
-    using Addr = SmemAddr<1>;
-    using First = Pass<M, 0, +1, NT, 1>;
-    using Last = Pass<M, Plan::npass - 1, +1, NT, 1>;
-    extern __shared__ float2 smem[];
-    float2 *X = smem;                 // [2][M] the channel's spectrum, both pols
-    float2 *ex = smem + 2 * M;        // exchange buffer, Addr::size(M)
-    const int tid = threadIdx.x;
-    const int c = blockIdx.x % nchan;
-    const int ulocal = blockIdx.x / nchan;
-    const int unit = unit0 + ulocal, b = unit / nsub, s = unit % nsub;
-
-    // channel spectrum -> shared memory (read from HBM once per DM tile)
-    {
-        const float4 *src0 = reinterpret_cast<const float4 *>(spec + ((size_t)ulocal * 2) * nfft + (size_t)c * M);
-        const float4 *src1 = reinterpret_cast<const float4 *>(spec + ((size_t)ulocal * 2 + 1) * nfft + (size_t)c * M);
-        float4 *d0 = reinterpret_cast<float4 *>(X), *d1 = reinterpret_cast<float4 *>(X + M);
-        for (int e = tid; e < M / 2; e += NT) {
-            d0[e] = __ldg(src0 + e);
-            d1[e] = __ldg(src1 + e);
-        }
-    }
-
-    // Eq. 1 per bin this thread feeds to pass 0: phase = DM * g, g in cycles per unit DM
-    double g[16];
-    {
-        const double fc = fcen[s];
-        const double df = bw_mhz / (double)nfft;
-        double f0;
-        if (chirp_ref == 0) f0 = fc + ((double)c + 0.5 - 0.5 * (double)nchan) * bw_mhz / (double)nchan;
-        else f0 = fc;
-#pragma unroll
-        for (int r = 0; r < 16; ++r) {
-            const int m = First::in_elem(tid, 0, r);
-            const double f = (chirp_ref == 0) ? (double)(m - M / 2) * df : (double)(c * M + m - nfft / 2) * df;
-            g[r] = f * f / (2.41e-10 * f0 * f0 * (f0 + f));
-        }
-    }
-    __syncthreads();
-
-    const int nchan_total = nsub * nchan;
-    const int ochan = nchan_total - 1 - (s * nchan + c);
-    const int d_begin = blockIdx.y * dm_tile;
-    const int d_end = min(ndm, d_begin + dm_tile);
-
-    for (int d = d_begin; d < d_end; ++d) {
-        const double dm = dmlist[d];
-        float2 H[16];
-#pragma unroll
-        for (int r = 0; r < 16; ++r) {
-            const double t = fma(dm, g[r], 6755399441055744.0);   // 1.5 * 2^52: round to nearest integer
-            const double n = t - 6755399441055744.0;
-            const float fr = (float)fma(dm, g[r], -n);            // in [-0.5, 0.5]
-            H[r] = unit_phasor<ACCURATE>(fr);
-        }
-        float acc[16];
-#pragma unroll
-        for (int i = 0; i < 16; ++i) acc[i] = 0.f;
-
-#pragma unroll 1
-        for (int p = 0; p < 2; ++p) {
-            float2 v[16];
-#pragma unroll
-            for (int r = 0; r < 16; ++r) v[r] = cmul(X[p * M + First::in_elem(tid, 0, r)], H[r]);
-            __syncthreads();  // the exchange buffer is free (previous transform / decimation done)
-            fft_passes<M, 0, +1, NT, 1, true>(v, ex, tw, tid);
-#pragma unroll
-            for (int i = 0; i < 16; ++i) acc[i] = fmaf(v[i].x, v[i].x, fmaf(v[i].y, v[i].y, acc[i]));
-        }
-
-        float *outd = out + (size_t)d * (size_t)out_stride_dm + (size_t)b * vdec * nchan_total + ochan;
-        if (FASTDEC) {
-            // ndec consecutive samples sit in ndec adjacent lanes
-#pragma unroll
-            for (int i = 0; i < 16; ++i) {
-                float a = acc[i];
-                for (int o = ndec >> 1; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
-                acc[i] = a;
-            }
-            if ((tid & (ndec - 1)) == 0) {
-#pragma unroll
-                for (int u = 0; u < Last::U; ++u)
-#pragma unroll
-                    for (int q = 0; q < Last::R; ++q) {
-                        const int t = Last::out_elem(tid, u, q);
-                        if (t >= hdisc && t < M - hdisc)
-                            outd[(size_t)((t - hdisc) / ndec) * nchan_total] = acc[u * Last::R + q] * scale;
-                    }
-            }
-        } else {
-            float *I = reinterpret_cast<float *>(ex);
-            __syncthreads();
-#pragma unroll
-            for (int u = 0; u < Last::U; ++u)
-#pragma unroll
-                for (int q = 0; q < Last::R; ++q) I[Last::out_elem(tid, u, q)] = acc[u * Last::R + q];
-            __syncthreads();
-            for (int qd = tid; qd < vdec; qd += NT) {
-                float a = 0.f;
-                for (int r = 0; r < ndec; ++r) a += I[hdisc + qd * ndec + r];
-                outd[(size_t)qd * nchan_total] = a * scale;
-            }
-        }
-    }
-}
-
-// ------------------------------------------------------------------------------------
 // FP32 FMA rate (roofline denominator)
 // ------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(1024) k_fp32_peak(float *out, int inner)
@@ -469,64 +338,6 @@ cudaError_t launch_forward(const Geometry &g, const Workspace &ws, const void *d
     if (e != cudaSuccess) return e;
     ++*launches;
     return cudaSuccess;
-}
-
-template <int M>
-static cudaError_t launch_fused_M(const Geometry &g, const Workspace &ws, const float2 *spec, int unit0, int nunits,
-                                  float *d_out, long long out_stride_dm, int dm_tile, int accurate, cudaStream_t st)
-{
-    constexpr int NT = M / 16;
-    const size_t smem = sizeof(float2) * (2 * (size_t)M + SmemAddr<1>::size(M));
-    const int D = g.ndec;
-    const bool fast = NT >= 32 && D <= 32 && (D & (D - 1)) == 0 && (g.hdisc % D) == 0;
-    if (dm_tile <= 0 || dm_tile > g.ndm) dm_tile = g.ndm;
-    dim3 grid((unsigned)(nunits * g.nchan), (unsigned)((g.ndm + dm_tile - 1) / dm_tile));
-    const float scale = (float)(1.0 / ((double)g.nfft * (double)M));
-    cudaError_t e;
-#define CDMT_FUSED(FAST, ACC)                                                                                        \
-    do {                                                                                                             \
-        e = cudaFuncSetAttribute(k_fused<M, FAST, ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);     \
-        if (e != cudaSuccess) return e;                                                                              \
-        k_fused<M, FAST, ACC><<<grid, NT, smem, st>>>(spec, ws.tw_m, ws.dm, ws.fcen, d_out, out_stride_dm, unit0,    \
-                                                      g.nsub, g.nchan, g.nfft, g.hdisc, g.ndec, g.vdec, g.ndm,       \
-                                                      dm_tile, g.chirp_ref, g.bw_mhz, scale);                        \
-    } while (0)
-    if (fast) {
-        if (accurate) CDMT_FUSED(true, true);
-        else CDMT_FUSED(true, false);
-    } else {
-        if (accurate) CDMT_FUSED(false, true);
-        else CDMT_FUSED(false, false);
-    }
-#undef CDMT_FUSED
-    return cudaGetLastError();
-}
-
-cudaError_t launch_fused(const Geometry &g, const Workspace &ws, const float2 *spec, int unit0, int nunits,
-                         float *d_out, long long out_stride_dm, int dm_tile, int accurate, cudaStream_t st,
-                         long long *launches)
-{
-    cudaError_t e;
-    switch (g.mbin) {
-#define CDMT_CASE(MM)                                                                                      \
-    case MM:                                                                                               \
-        e = launch_fused_M<MM>(g, ws, spec, unit0, nunits, d_out, out_stride_dm, dm_tile, accurate, st);   \
-        break;
-        CDMT_CASE(16)
-        CDMT_CASE(32)
-        CDMT_CASE(64)
-        CDMT_CASE(128)
-        CDMT_CASE(256)
-        CDMT_CASE(512)
-        CDMT_CASE(1024)
-        CDMT_CASE(2048)
-        CDMT_CASE(4096)
-        CDMT_CASE(8192)
-#undef CDMT_CASE
-    default: return cudaErrorInvalidValue;
-    }
-    if (e == cudaSuccess) ++*launches;
-    return e;
 }
 
 }  // namespace cdmt
