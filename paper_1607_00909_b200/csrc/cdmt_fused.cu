@@ -14,6 +14,8 @@
 //                          integration; <= 128 registers so that two CTAs share an SM at M = 4096.
 //  k_fused_generic<M>      any ndec / overlap / M >= 16: exact per-bin phase constants in
 //                          registers, autosort passes, integration through shared memory.
+#include <cstdint>
+
 #include "cdmt_fft.cuh"
 #include "cdmt_internal.h"
 
@@ -46,6 +48,12 @@ __device__ __forceinline__ float frac_cycles(double dm, double g)
     return (float)fma(dm, g, -n);
 }
 
+constexpr int DM_PARAM_MAX = 1024;  // DM trials carried in the kernel parameter block (constant bank)
+
+struct DmParams {
+    double dm[DM_PARAM_MAX];
+};
+
 struct FusedArgs {
     const float2 *spec;      // [units][2][nfft] swapped-halves spectra of this chunk
     const float2 *tw;        // pass twiddles of the length-M backward transform
@@ -54,6 +62,7 @@ struct FusedArgs {
     float *out;
     long long out_stride_dm;
     int unit0, nsub, nchan, nfft, hdisc, ndec, vdec, ndm, dm_tile, chirp_ref, accurate;
+    int dm_first, dm_param0;  // DM range [dm_first, ndm) of this launch; dmp.dm[0] is trial dm_param0
     double bw_mhz;
     float scale;
 };
@@ -112,7 +121,7 @@ __global__ void __launch_bounds__(M / 16) k_fused_generic(const FusedArgs a)
     __syncthreads();
     const int nchan_total = a.nsub * a.nchan;
     const int ochan = nchan_total - 1 - (s * a.nchan + c);
-    const int d_begin = blockIdx.y * a.dm_tile;
+    const int d_begin = a.dm_first + blockIdx.y * a.dm_tile;
     const int d_end = min(a.ndm, d_begin + a.dm_tile);
     for (int d = d_begin; d < d_end; ++d) {
         const double dm = a.dmlist[d];
@@ -149,70 +158,87 @@ __global__ void __launch_bounds__(M / 16) k_fused_generic(const FusedArgs a)
 }
 
 // ------------------------------------------------------------------------------------
-// fast kernel: in-place passes.  Digits: pass p transforms input digit i_p (stride M/(R_0..R_p))
-// into output digit o_p (weight T_p = R_0..R_(p-1)).  A value with digits (d_0, d_1, ..)
-// lives at d_0 * (M/16 + 1) + sum_{q>=1} d_q A_q, A_q = product of the radices after q; the
-// odd pitch of d_0 makes every access of 16 consecutive d_0 bank-conflict free.
+// fast kernel: in-place passes.  Pass p transforms input digit i_p (stride M/(R_0..R_p)) into
+// output digit o_p (weight T_p = R_0..R_(p-1)); a value whose digits are (d_0, d_1, rho), rho =
+// the remaining digits in natural order, lives at rho*16*PITCH + d_1*PITCH + d_0:
+//   pass 0: thread (rho, d_1) writes its 16 outputs d_0 = 0..15 as 8 consecutive 16-byte words
+//   pass 1: thread (rho, d_0) reads/writes d_1 = 0..15 -- the same 16 threads (one half-warp)
+//           that wrote them, so a __syncwarp() is all that pass 0 -> pass 1 needs
+//   pass p>=2: lanes run over d_0 (consecutive addresses), block barrier before it
+// The barrier that protects the buffer against the NEXT transform's pass-0 stores is split
+// into an mbarrier arrive (after the last pass has read) and a wait (before pass 0 stores).
 // ------------------------------------------------------------------------------------
 template <int M>
 struct InplacePlan {
     using Plan = RadixPlan<M>;
     static constexpr int NT = M / 16;
-    static constexpr int A0 = M / 16 + 1;
-    static constexpr int size = 16 * A0;
+    static constexpr int PITCH = 18;                    // d_1 pitch in elements: 16-byte aligned, 4 banks apart
+    static constexpr int RHO = 16 * PITCH;              // elements per rho
+    static constexpr int size = (M / 256) * RHO;
     static constexpr int after(int p)  // product of radices after pass p
     {
         int n = 1;
         for (int q = p + 1; q < Plan::npass; ++q) n *= Plan::radix(q);
         return n;
     }
+    // the bin offset (within its radix-16 column) that pass-0 thread t owns
+    static __device__ __forceinline__ int rest_of_thread(int t) { return (t & 15) * (NT / 16) + (t >> 4); }
 };
 
 template <int M, int P>
 struct InplacePass {
+    static_assert(P >= 1, "pass 0 is written out in the kernel");
     using Plan = RadixPlan<M>;
     using IP = InplacePlan<M>;
     static constexpr int NT = IP::NT;
     static constexpr int R = Plan::radix(P);
     static constexpr int T = Plan::ns(P);     // weight of the output digit
-    static constexpr int A = IP::after(P);    // address stride of the digit
+    static constexpr int A = IP::after(P);    // stride of digit P inside rho (P >= 2)
+    static constexpr int A2 = IP::after(2);
     static constexpr int U = 16 / R;
     static constexpr int TWOFF = Plan::tw_offset(P);
-    static constexpr int A1 = IP::after(1);
-    static constexpr int A2 = IP::after(2);
+    static constexpr int XSTRIDE = (P == 1) ? IP::PITCH : A * IP::RHO;
 
-    // shared-memory address of element x = 0 of butterfly beta
-    static __device__ __forceinline__ int base(int beta)
+    // twiddle index K of butterfly beta and the address of its element x = 0
+    static __device__ __forceinline__ void decode(int beta, int *K, int *base)
     {
-        const int K = beta % T, lo = beta / T;
-        int addr = (K & 15) * IP::A0 + lo;
-        if (P >= 2) addr += ((K >> 4) & 15) * A1;
-        if (P >= 3) addr += ((K >> 8) & 15) * A2;
-        return addr;
+        if (P == 1) {  // beta = rho*16 + d0
+            *K = beta & 15;
+            *base = (beta >> 4) * IP::RHO + (beta & 15);
+        } else {       // beta = K + T*lo, K = d0 + 16 d1 (+ 256 d2)
+            const int k = beta % T, lo = beta / T;
+            int rho = lo;
+            if (P >= 3) rho += ((k >> 8) & 15) * A2;
+            *K = k;
+            *base = rho * IP::RHO + ((k >> 4) & 15) * IP::PITCH + (k & 15);
+        }
     }
     static __device__ __forceinline__ void load(const float2 *ex, float2 *v, int tid)
     {
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            const int bs = base(tid + u * NT);
+            int K, bs;
+            decode(tid + u * NT, &K, &bs);
 #pragma unroll
-            for (int x = 0; x < R; ++x) v[u * R + x] = ex[bs + x * A];
+            for (int x = 0; x < R; ++x) v[u * R + x] = ex[bs + x * XSTRIDE];
         }
     }
     static __device__ __forceinline__ void store(float2 *ex, const float2 *v, int tid)
     {
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            const int bs = base(tid + u * NT);
+            int K, bs;
+            decode(tid + u * NT, &K, &bs);
 #pragma unroll
-            for (int x = 0; x < R; ++x) ex[bs + x * A] = v[u * R + x];
+            for (int x = 0; x < R; ++x) ex[bs + x * XSTRIDE] = v[u * R + x];
         }
     }
     static __device__ __forceinline__ void compute(float2 *v, const float2 *__restrict__ tw, int tid)
     {
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            const int K = (tid + u * NT) % T;
+            int K, bs;
+            decode(tid + u * NT, &K, &bs);
             const float2 *t = tw + TWOFF + K;
 #pragma unroll
             for (int x = 1; x < R; ++x) v[u * R + x] = cmul(v[u * R + x], __ldg(t + (x - 1) * T));
@@ -221,16 +247,43 @@ struct InplacePass {
     }
 };
 
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(
+                     (unsigned)__cvta_generic_to_shared(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tWAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}" ::"r"((unsigned)__cvta_generic_to_shared(bar)),
+        "r"(parity)
+        : "memory");
+}
+
+// passes 2.. : block barrier, load, butterfly, (store in place)
 template <int M, int P>
-__device__ __forceinline__ void inplace_tail(float2 *v, float2 *ex, const float2 *__restrict__ tw, int tid)
+__device__ __forceinline__ void inplace_tail(float2 *v, float2 *ex, const float2 *__restrict__ tw, int tid,
+                                             uint64_t *bar)
 {
     using Ps = InplacePass<M, P>;
     __syncthreads();  // previous pass stored
     Ps::load(ex, v, tid);
-    Ps::compute(v, tw, tid);
-    if constexpr (P + 1 < RadixPlan<M>::npass) {
+    if constexpr (P + 1 == RadixPlan<M>::npass) {
+        // the multiply below depends on every load above: once it has issued, the buffer may
+        // be overwritten by the next transform
+        Ps::compute(v, tw, tid);
+        mbar_arrive(bar);
+    } else {
+        Ps::compute(v, tw, tid);
         Ps::store(ex, v, tid);  // same slots this thread just read
-        inplace_tail<M, P + 1>(v, ex, tw, tid);
+        inplace_tail<M, P + 1>(v, ex, tw, tid, bar);
     }
 }
 
@@ -255,7 +308,7 @@ __device__ __forceinline__ void lane_reduce_scatter(float *a, int lane)
 
 template <int M, int LOGD>
 __global__ void __launch_bounds__(M / 16, (512 / (M / 16) > 16 ? 16 : (512 / (M / 16) < 1 ? 1 : 512 / (M / 16))))
-k_fused_fast(const FusedArgs a)
+k_fused_fast(const FusedArgs a, const __grid_constant__ DmParams dmp)
 {
     constexpr int NT = M / 16;
     constexpr int D = 1 << LOGD;
@@ -263,54 +316,64 @@ k_fused_fast(const FusedArgs a)
     constexpr int NKEEP = 16 >> LS;          // integrated samples per thread per DM
     using Plan = RadixPlan<M>;
     using IP = InplacePlan<M>;
+    using P1 = InplacePass<M, 1>;
     using LastP = InplacePass<M, Plan::npass - 1>;
-    static_assert(Plan::npass >= 2 && NT >= 32, "fast path needs M >= 512");
+    static_assert(Plan::npass >= 3 && NT >= 32, "fast path needs M >= 512");
     extern __shared__ float2 smem[];
-    float2 *X = smem;           // [2][M]
+    float2 *X = smem;           // [2][16][NT]: bin x NT + rest(t) at [x][t]
     float2 *ex = smem + 2 * M;  // IP::size
+    double *coef = reinterpret_cast<double *>(ex + IP::size);  // [6][NT]
+    uint64_t *bar = reinterpret_cast<uint64_t *>(coef + 6 * NT);
     const int tid = threadIdx.x;
     const int lane = tid & 31;
     const int c = blockIdx.x % a.nchan;
     const int ulocal = blockIdx.x / a.nchan;
     const int unit = a.unit0 + ulocal, b = unit / a.nsub, s = unit % a.nsub;
+    if (tid == 0) mbar_init(bar, NT);
     {
-        const float4 *src0 = reinterpret_cast<const float4 *>(a.spec + ((size_t)ulocal * 2) * a.nfft + (size_t)c * M);
-        const float4 *src1 = reinterpret_cast<const float4 *>(a.spec + ((size_t)ulocal * 2 + 1) * a.nfft + (size_t)c * M);
-        float4 *d0 = reinterpret_cast<float4 *>(X), *d1 = reinterpret_cast<float4 *>(X + M);
+        // channel spectrum -> shared memory in the order pass 0 reads it
+        const float2 *src0 = a.spec + ((size_t)ulocal * 2) * a.nfft + (size_t)c * M;
+        const float2 *src1 = src0 + a.nfft;
 #pragma unroll 4
-        for (int e = tid; e < M / 2; e += NT) {
-            d0[e] = __ldg(src0 + e);
-            d1[e] = __ldg(src1 + e);
+        for (int m = tid; m < M; m += NT) {
+            const int x = m / NT, rest = m % NT;
+            const int t = (rest % (NT / 16)) * 16 + rest / (NT / 16);
+            X[x * NT + t] = __ldg(src0 + m);
+            X[M + x * NT + t] = __ldg(src1 + m);
         }
     }
-    // Eq. 1 along this thread's bins m_r = tid + r M/16: g(f_a + b r) = sum_k ck r^k (Taylor in
-    // b r / (f0 + f_a) <= 1e-3; the host checks that the r^6 term is below 1e-7 cycles)
-    double c0, c1, c2, c3, c4, c5;
+    // Eq. 1 along this thread's bins m_r = rest + r M/16: g(f_a + b r) = sum_k ck r^k (Taylor in
+    // b r / (f0 + f_a) <= 1e-3; the host checks that the r^6 term is below 1e-7 cycles).
     {
         double f0, fb0, df;
         chirp_axes(a, s, c, M, &f0, &fb0, &df);
-        const double fa = fb0 + (double)tid * df, bb = (double)NT * df;
+        const double fa = fb0 + (double)IP::rest_of_thread(tid) * df, bb = (double)NT * df;
         const double kc = 1.0 / (2.41e-10 * f0 * f0);
         const double sa = f0 + fa, e = bb / sa, pp = kc * f0 * f0 / sa;
-        c0 = kc * fa * fa / sa;
-        c1 = kc * (fa * fa + 2.0 * fa * f0) / (sa * sa) * bb;
-        c2 = pp * e * e;
-        c3 = -c2 * e;
-        c4 = -c3 * e;
-        c5 = -c4 * e;
+        const double c2 = pp * e * e, c3 = -c2 * e, c4 = -c3 * e, c5 = -c4 * e;
+        coef[0 * NT + tid] = kc * fa * fa / sa;
+        coef[1 * NT + tid] = kc * (fa * fa + 2.0 * fa * f0) / (sa * sa) * bb;
+        coef[2 * NT + tid] = c2;
+        coef[3 * NT + tid] = c3;
+        coef[4 * NT + tid] = c4;
+        coef[5 * NT + tid] = c5;
     }
     const int nchan_total = a.nsub * a.nchan;
     const int ochan = nchan_total - 1 - (s * a.nchan + c);
     float *out0 = a.out + (size_t)b * a.vdec * nchan_total + ochan;
-    const int d_begin = blockIdx.y * a.dm_tile;
+    const int d_begin = a.dm_first + blockIdx.y * a.dm_tile;
     const int d_end = min(a.ndm, d_begin + a.dm_tile);
+    // pass-0 thread (rho, d1) = (tid >> 4, tid & 15) stores at rho*RHO + d1*PITCH + 0..15
+    float4 *p0_store = reinterpret_cast<float4 *>(ex + (tid >> 4) * IP::RHO + (tid & 15) * IP::PITCH);
+    unsigned nfft_done = 0;  // transforms finished by this CTA: parity of the mbarrier phase
     __syncthreads();
 
 #pragma unroll 1
     for (int d = d_begin; d < d_end; ++d) {
-        const double dm = a.dmlist[d];
+        const double dm = dmp.dm[d - a.dm_param0];
         // phase polynomial of this DM (scaling the coefficients keeps the evaluation inside the loop)
-        const double p0 = dm * c0, p1 = dm * c1, p2 = dm * c2, p3 = dm * c3, p4 = dm * c4, p5 = dm * c5;
+        const double p0 = dm * coef[0 * NT + tid], p1 = dm * coef[1 * NT + tid], p2 = dm * coef[2 * NT + tid];
+        const double p3 = dm * coef[3 * NT + tid], p4 = dm * coef[4 * NT + tid], p5 = dm * coef[5 * NT + tid];
         float2 H[16];
 #pragma unroll
         for (int r = 0; r < 16; ++r) {
@@ -325,12 +388,18 @@ k_fused_fast(const FusedArgs a)
         for (int p = 0; p < 2; ++p) {
             float2 v[16];
 #pragma unroll
-            for (int r = 0; r < 16; ++r) v[r] = cmul(X[p * M + tid + r * NT], H[r]);
+            for (int r = 0; r < 16; ++r) v[r] = cmul(X[p * M + r * NT + tid], H[r]);
             Dft<16, +1>::run(v);
-            __syncthreads();  // every thread has finished reading the previous transform
+            if (nfft_done) mbar_wait(bar, (nfft_done - 1) & 1);  // previous transform fully read
 #pragma unroll
-            for (int q = 0; q < 16; ++q) ex[q * IP::A0 + tid] = v[q];
-            inplace_tail<M, 1>(v, ex, a.tw, tid);
+            for (int q = 0; q < 8; ++q)
+                p0_store[q] = make_float4(v[2 * q].x, v[2 * q].y, v[2 * q + 1].x, v[2 * q + 1].y);
+            __syncwarp();
+            P1::load(ex, v, tid);
+            P1::compute(v, a.tw, tid);
+            P1::store(ex, v, tid);
+            inplace_tail<M, 2>(v, ex, a.tw, tid, bar);
+            ++nfft_done;
             // v[u R + x] = y[t], t = tid + NT (u + U x): reorder to n = u + U x, detect
             float pw[16];
 #pragma unroll
@@ -370,25 +439,40 @@ static cudaError_t launch_generic_M(const FusedArgs &fa, dim3 grid, cudaStream_t
 }
 
 template <int M, int LOGD>
-static cudaError_t launch_fast_MD(const FusedArgs &fa, dim3 grid, cudaStream_t st)
+static cudaError_t launch_fast_MD(FusedArgs fa, const double *h_dm, int nunits, cudaStream_t st, long long *launches)
 {
-    const size_t smem = sizeof(float2) * (2 * (size_t)M + InplacePlan<M>::size);
+    const size_t smem = sizeof(float2) * (2 * (size_t)M + InplacePlan<M>::size) + sizeof(double) * 6 * (M / 16) + 16;
     cudaError_t e = cudaFuncSetAttribute(k_fused_fast<M, LOGD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_fused_fast<M, LOGD><<<grid, M / 16, smem, st>>>(fa);
-    return cudaGetLastError();
+    const int ndm_total = fa.ndm;
+    for (int d0 = 0; d0 < ndm_total; d0 += DM_PARAM_MAX) {
+        const int cnt = ndm_total - d0 < DM_PARAM_MAX ? ndm_total - d0 : DM_PARAM_MAX;
+        DmParams dmp;
+        for (int i = 0; i < cnt; ++i) dmp.dm[i] = h_dm[d0 + i];
+        for (int i = cnt; i < DM_PARAM_MAX; ++i) dmp.dm[i] = 0.0;
+        fa.dm_first = d0;
+        fa.dm_param0 = d0;
+        fa.ndm = d0 + cnt;
+        dim3 grid((unsigned)(nunits * fa.nchan), (unsigned)((cnt + fa.dm_tile - 1) / fa.dm_tile));
+        k_fused_fast<M, LOGD><<<grid, M / 16, smem, st>>>(fa, dmp);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+        ++*launches;
+    }
+    return cudaSuccess;
 }
 
 template <int M>
-static cudaError_t launch_fast_M(int logd, const FusedArgs &fa, dim3 grid, cudaStream_t st)
+static cudaError_t launch_fast_M(int logd, const FusedArgs &fa, const double *h_dm, int nunits, cudaStream_t st,
+                                 long long *launches)
 {
     switch (logd) {
-    case 0: return launch_fast_MD<M, 0>(fa, grid, st);
-    case 1: return launch_fast_MD<M, 1>(fa, grid, st);
-    case 2: return launch_fast_MD<M, 2>(fa, grid, st);
-    case 3: return launch_fast_MD<M, 3>(fa, grid, st);
-    case 4: return launch_fast_MD<M, 4>(fa, grid, st);
-    case 5: return launch_fast_MD<M, 5>(fa, grid, st);
+    case 0: return launch_fast_MD<M, 0>(fa, h_dm, nunits, st, launches);
+    case 1: return launch_fast_MD<M, 1>(fa, h_dm, nunits, st, launches);
+    case 2: return launch_fast_MD<M, 2>(fa, h_dm, nunits, st, launches);
+    case 3: return launch_fast_MD<M, 3>(fa, h_dm, nunits, st, launches);
+    case 4: return launch_fast_MD<M, 4>(fa, h_dm, nunits, st, launches);
+    case 5: return launch_fast_MD<M, 5>(fa, h_dm, nunits, st, launches);
     default: return cudaErrorInvalidValue;
     }
 }
@@ -418,6 +502,8 @@ cudaError_t launch_fused(const Geometry &g, const Workspace &ws, const float2 *s
     fa.hdisc = g.hdisc; fa.ndec = g.ndec; fa.vdec = g.vdec; fa.ndm = g.ndm; fa.dm_tile = dm_tile;
     fa.chirp_ref = g.chirp_ref; fa.accurate = accurate; fa.bw_mhz = g.bw_mhz;
     fa.scale = (float)(1.0 / ((double)g.nfft * (double)M));
+    fa.dm_first = 0;
+    fa.dm_param0 = 0;
     int logd = 0;
     while ((1 << logd) < D) ++logd;
     const bool fast = !force_generic && !accurate && M >= 512 && D <= 32 && (1 << logd) == D && (g.hdisc % D) == 0 &&
@@ -425,13 +511,14 @@ cudaError_t launch_fused(const Geometry &g, const Workspace &ws, const float2 *s
     cudaError_t e = cudaErrorInvalidValue;
     if (fast) {
         switch (M) {
-        case 512: e = launch_fast_M<512>(logd, fa, grid, st); break;
-        case 1024: e = launch_fast_M<1024>(logd, fa, grid, st); break;
-        case 2048: e = launch_fast_M<2048>(logd, fa, grid, st); break;
-        case 4096: e = launch_fast_M<4096>(logd, fa, grid, st); break;
-        case 8192: e = launch_fast_M<8192>(logd, fa, grid, st); break;
+        case 512: e = launch_fast_M<512>(logd, fa, h_dm, nunits, st, launches); break;
+        case 1024: e = launch_fast_M<1024>(logd, fa, h_dm, nunits, st, launches); break;
+        case 2048: e = launch_fast_M<2048>(logd, fa, h_dm, nunits, st, launches); break;
+        case 4096: e = launch_fast_M<4096>(logd, fa, h_dm, nunits, st, launches); break;
+        case 8192: e = launch_fast_M<8192>(logd, fa, h_dm, nunits, st, launches); break;
         default: break;
         }
+        return e;
     } else {
         switch (M) {
         case 16: e = launch_generic_M<16>(fa, grid, st); break;
