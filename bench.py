@@ -59,6 +59,22 @@ def rank_workload(cfg: synth.Config, rank: int, world: int) -> synth.Config:
     return cfg
 
 
+def max_over_ranks(value: float, world: int, device=None) -> float:
+    """MAX all-reduce of a per-rank scalar (device time); identity for one rank."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(cfg: synth.Config, world: int, sec_per_step: float) -> float:
+    """Metric over all ranks: every rank processed nsub*nsamp samples x ndm trials per step."""
+    return world * float(cfg.nsub) * cfg.nsamp * cfg.ndm / sec_per_step
+
+
 class ClockSampler:
     """nvidia-smi clocks and throttle reasons during the timed region."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -110,16 +126,22 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def oracle_sample(cfg: synth.Config, nunits: int, x_sub0: np.ndarray):
-    """Time the oracle, as it stands, on `nunits` (subband 0, block b) units with every DM."""
+def oracle_sample(cfg: synth.Config, nunits: int, xsubs):
+    """Time the oracle, as it stands, on `nunits` (subband, block) units with every DM trial.
+    xsubs: list of generated subbands 0..k; units are taken block by block, subband by subband."""
     from oracle import cdmt_oracle as orc
     p = orc.Params(**cfg.plan_kwargs())
-    blocks = np.stack([x_sub0[:, b * cfg.step:b * cfg.step + cfg.nfft] for b in range(nunits)])
+    us = [(i // cfg.nblock, i % cfg.nblock) for i in range(nunits)]
+    blocks = np.stack([xsubs[s][:, b * cfg.step:b * cfg.step + cfg.nfft] for s, b in us])
     t0 = time.perf_counter()
-    orc.units(p, [0] * nunits, blocks)
+    orc.units(p, [s for s, _ in us], blocks)
     dt = time.perf_counter() - t0
     samples_dm = nunits / float(cfg.nsub * cfg.nblock) * cfg.nsub * cfg.nsamp * cfg.ndm
     return samples_dm / dt, dt, orc.num_threads()
+
+
+def oracle_sample_size(cfg: synth.Config, ncores: int, per_core: int) -> int:
+    return max(1, min(cfg.nsub * cfg.nblock, per_core * ncores))
 
 
 def run_reference(args, cfg, rank, world):
@@ -128,14 +150,14 @@ def run_reference(args, cfg, rank, world):
         return
     from oracle import cdmt_oracle as orc
     ncores = orc.num_threads()
-    x0 = synth.generate_subband(cfg, 0)
-    nunits = min(cfg.nblock, max(1, ncores))
+    nunits = oracle_sample_size(cfg, ncores, 2)
+    xs = [synth.generate_subband(cfg, s) for s in range((nunits + cfg.nblock - 1) // cfg.nblock)]
     for _ in range(args.warmup):
-        oracle_sample(cfg, min(nunits, 2), x0)
+        oracle_sample(cfg, min(nunits, ncores), xs)
     t0 = time.perf_counter()
     done = 0.0
     for _ in range(args.steps):
-        rate, dt, _ = oracle_sample(cfg, nunits, x0)
+        rate, dt, _ = oracle_sample(cfg, nunits, xs)
         done += rate * dt
     total = time.perf_counter() - t0
     value = done / total
@@ -289,13 +311,10 @@ def main():
     clocks = sampler.stop()
     prof = cdmt.cdmt_profile_read(plan)
     cdmt.cdmt_plan_set_option(plan, cdmt.OPT_PROFILE, 0)
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, world, dev)
     sec_per_step = ms * 1e-3 / args.steps
     samples_dm = float(cfg.nsub) * cfg.nsamp * cfg.ndm
-    value = world * samples_dm / sec_per_step
+    value = whole_job_value(cfg, world, sec_per_step)
 
     # ---- roofline of the dominant kernel (fused per-DM kernel): ALU bound
     units_per_step = cfg.nsub * nb_total
@@ -331,12 +350,9 @@ def main():
             cdmt.cdmt_execute_host(plan, h_in.data_ptr(), cfg.nsamp, cfg.nsamp, h_out.data_ptr(), d_scr, nbytes, stream)
         torch.cuda.synchronize()
         dt = (time.perf_counter() - t0) / ksteps
-        if world > 1:
-            t = torch.tensor([dt], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = max_over_ranks(dt, world, dev)
         esz = 2 if int8 else 8
-        e2e = {"value": world * samples_dm / dt, "unit": UNIT,
+        e2e = {"value": whole_job_value(cfg, world, dt), "unit": UNIT,
                "h2d_bytes_per_step": int(cfg.nsub * 2 * q["nsamp_consumed"] * esz),
                "d2h_bytes_per_step": int(q["out_bytes"]), "ms_per_step": dt * 1e3, "steps": ksteps,
                "api": "cdmt_execute_host (pinned host in/out)"}
@@ -347,8 +363,9 @@ def main():
     if rank == 0 and world == 1 and not args.no_cpu:
         from oracle import cdmt_oracle as orc
         ncores = orc.num_threads()
-        nun = min(cfg.nblock, max(1, ncores))
-        rate, dt, ncores = oracle_sample(cfg, nun, x_sub0)
+        nun = oracle_sample_size(cfg, ncores, 14)       # about 10-30 s of CPU work
+        xs = [x_sub0] + [synth.generate_subband(cfg, s) for s in range(1, (nun + cfg.nblock - 1) // cfg.nblock)]
+        rate, dt, ncores = oracle_sample(cfg, nun, xs)
         cpu = {"value": rate, "unit": UNIT, "cores": ncores, "kind": "oracle", "seconds": dt,
                "sample": "%d of %d (subband, block) units of %s x all %d DMs" % (
                    nun, cfg.nsub * cfg.nblock, cfg.name, cfg.ndm)}

@@ -1,0 +1,88 @@
+"""Host-side logic of bench.py (no GPU): flop accounting, the N>1 reduction over gloo with
+world_size 2, and the reference arm launched the way the driver launches it."""
+import json
+import os
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+sys.path.insert(0, ROOT)
+
+import bench  # noqa: E402
+from paper_1607_00909_b200 import synth  # noqa: E402
+
+
+def test_flop_accounting_matches_scope_table():
+    # per-unit per-DM flops c2 11.08, c3 10.35, c4 43.5, c5 10.88 MF
+    for name, mf in (("c2", 11.08), ("c3", 10.35), ("c4", 43.5), ("c5", 10.88)):
+        got = bench.algorithmic_flops_per_unit_dm(synth.make_config(name)) / 1e6
+        assert abs(got - mf) < 0.06, (name, got)
+    # c3 total 12.2 TF
+    c3 = synth.make_config("c3")
+    tot = bench.algorithmic_flops_per_unit_dm(c3) * c3.ndm * c3.nsub * c3.nblock
+    assert abs(tot / 1e12 - 12.0) < 0.3
+    assert abs(bench.FP32_PEAK_TFLOPS - 74.45) < 0.01
+
+
+def test_rank_workloads_differ_only_by_seed():
+    a = bench.rank_workload(synth.make_config("c1"), 0, 2)
+    b = bench.rank_workload(synth.make_config("c1"), 1, 2)
+    assert a.seed != b.seed and a.nsub == b.nsub and a.nsamp == b.nsamp
+    xa, xb = synth.generate(a), synth.generate(b)
+    assert xa.shape == xb.shape and not np.array_equal(xa, xb)
+    solo = bench.rank_workload(synth.make_config("c1"), 0, 1)
+    assert solo.seed == synth.make_config("c1").seed
+
+
+WORKER = r"""
+import os, sys, json
+sys.path.insert(0, %(root)r)
+import torch, torch.distributed as dist
+import bench
+from paper_1607_00909_b200 import synth
+dist.init_process_group("gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+cfg = bench.rank_workload(synth.make_config("c1"), rank, world)
+ms = 10.0 + 5.0 * rank                      # rank 1 is slower
+dist.barrier()
+mx = bench.max_over_ranks(ms, world)
+val = bench.whole_job_value(cfg, world, mx * 1e-3)
+if rank == 0:
+    print(json.dumps({"max_ms": mx, "value": val, "world": world}))
+dist.destroy_process_group()
+"""
+
+
+def _torchrun(args, timeout=600):
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", OMP_NUM_THREADS="2")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+           "--master-addr", "127.0.0.1", "--master-port", "29517"] + args
+    return subprocess.run(cmd, env=env, cwd=ROOT, capture_output=True, text=True, timeout=timeout)
+
+
+def test_max_over_ranks_gloo_world2(tmp_path):
+    script = tmp_path / "worker.py"
+    script.write_text(WORKER % {"root": ROOT})
+    r = _torchrun([str(script)])
+    assert r.returncode == 0, r.stderr[-2000:]
+    line = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(line) == 1
+    d = json.loads(line[0])
+    assert d["world"] == 2 and d["max_ms"] == 15.0
+    c1 = synth.make_config("c1")
+    assert abs(d["value"] - 2 * c1.nsub * c1.nsamp * c1.ndm / 15e-3) < 1e-3 * d["value"]
+
+
+def test_reference_arm_two_ranks_prints_one_line():
+    r = _torchrun(["bench.py", "--impl", "reference", "--gpus", "2", "--steps", "1", "--warmup", "1",
+                   "--config", "c1"])
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["metric"] == bench.METRIC and d["value"] > 0
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["e2e"]["h2d_bytes_per_step"] == 0
+    assert d["n_gpus"] == 2 and d["higher_is_better"] is True
