@@ -18,7 +18,7 @@ struct cdmt_plan {
     int dm_tile;             // 0 = all
     int accurate;
     int profile;             // record CUDA events around each kernel class
-    int force_generic;       // use k_fused_generic even where the fast kernel applies
+    int force_generic;       // CDMT_OPT_FUSED_KERNEL: 0 auto, 1 generic, 2 scalar fast, 3 packed
     long long last_launches;
     std::vector<cudaEvent_t> ev_pool;   // created lazily, reused
     size_t ev_used;
@@ -154,8 +154,8 @@ extern "C" int cdmt_plan_set_option(cdmt_plan *plan, int key, long long value)
         if (value != 0 && value != 1) return CDMT_ERR_ARG;
         plan->profile = (int)value;
         return CDMT_OK;
-    case CDMT_OPT_FORCE_GENERIC:
-        if (value != 0 && value != 1) return CDMT_ERR_ARG;
+    case CDMT_OPT_FUSED_KERNEL:
+        if (value < 0 || value > 3) return CDMT_ERR_ARG;
         plan->force_generic = (int)value;
         return CDMT_OK;
     default: return CDMT_ERR_ARG;

@@ -17,70 +17,10 @@
 #include <cstdint>
 
 #include "cdmt_fft.cuh"
+#include "cdmt_fused_common.cuh"
 #include "cdmt_internal.h"
 
 namespace cdmt {
-
-template <bool ACCURATE>
-__device__ __forceinline__ float2 unit_phasor(float frac_cycles)
-{
-    float s, c;
-    if (ACCURATE) {
-        sincospif(2.0f * frac_cycles, &s, &c);
-    } else {
-        const float x = frac_cycles * 6.283185307179586f;
-        s = __sinf(x);
-        c = __cosf(x);
-    }
-    return make_float2(c, s);
-}
-
-__device__ __forceinline__ float2 unit_phasor_rt(float frac_cycles, int accurate)
-{
-    return accurate ? unit_phasor<true>(frac_cycles) : unit_phasor<false>(frac_cycles);
-}
-
-// fractional part in [-0.5, 0.5] of dm * g, exact to fp64 rounding
-__device__ __forceinline__ float frac_cycles(double dm, double g)
-{
-    const double magic = 6755399441055744.0;  // 1.5 * 2^52: adding it rounds to the nearest integer
-    const double n = fma(dm, g, magic) - magic;
-    return (float)fma(dm, g, -n);
-}
-
-constexpr int DM_PARAM_MAX = 1024;  // DM trials carried in the kernel parameter block (constant bank)
-
-struct DmParams {
-    double dm[DM_PARAM_MAX];
-};
-
-struct FusedArgs {
-    const float2 *spec;      // [units][2][nfft] swapped-halves spectra of this chunk
-    const float2 *tw;        // pass twiddles of the length-M backward transform
-    const double *dmlist;
-    const double *fcen;
-    float *out;
-    long long out_stride_dm;
-    int unit0, nsub, nchan, nfft, hdisc, ndec, vdec, ndm, dm_tile, chirp_ref, accurate;
-    int dm_first, dm_param0;  // DM range [dm_first, ndm) of this launch; dmp.dm[0] is trial dm_param0
-    double bw_mhz;
-    float scale;
-};
-
-// frequency set-up shared by both kernels: nu_0 of Eq. 1 and the offset of bin m (MHz)
-__device__ __forceinline__ void chirp_axes(const FusedArgs &a, int s, int c, int M, double *f0, double *f_bin0,
-                                           double *df)
-{
-    const double fc = a.fcen[s];
-    *df = a.bw_mhz / (double)a.nfft;
-    if (a.chirp_ref == 0) {
-        *f0 = fc + ((double)c + 0.5 - 0.5 * (double)a.nchan) * a.bw_mhz / (double)a.nchan;
-        *f_bin0 = -(double)(M / 2) * *df;
-    } else {
-        *f0 = fc;
-        *f_bin0 = (double)(c * M - a.nfft / 2) * *df;
-    }
-}
 
 // ------------------------------------------------------------------------------------
 // generic kernel
@@ -246,26 +186,6 @@ struct InplacePass {
         }
     }
 };
-
-__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
-{
-    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(
-                     (unsigned)__cvta_generic_to_shared(bar))
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity)
-{
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tWAIT_%=:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-        "@p bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}" ::"r"((unsigned)__cvta_generic_to_shared(bar)),
-        "r"(parity)
-        : "memory");
-}
 
 // passes 2.. : block barrier, load, butterfly, (store in place)
 template <int M, int P>
@@ -506,8 +426,14 @@ cudaError_t launch_fused(const Geometry &g, const Workspace &ws, const float2 *s
     fa.dm_param0 = 0;
     int logd = 0;
     while ((1 << logd) < D) ++logd;
-    const bool fast = !force_generic && !accurate && M >= 512 && D <= 32 && (1 << logd) == D && (g.hdisc % D) == 0 &&
-                      poly_phase_ok(g, h_dm, h_fcen);
+    // force_generic carries CDMT_OPT_FUSED_KERNEL: 0 auto, 1 generic, 2 scalar fast, 3 packed (x2)
+    const bool fast_ok = !accurate && M >= 512 && D <= 32 && (1 << logd) == D && (g.hdisc % D) == 0 &&
+                         poly_phase_ok(g, h_dm, h_fcen);
+    const bool x2_ok = fast_ok && fused_x2_supported(M, D, g.hdisc);
+    if (force_generic == 3 && !x2_ok) return cudaErrorInvalidValue;
+    if (force_generic == 2 && !fast_ok) return cudaErrorInvalidValue;
+    if (x2_ok && (force_generic == 0 || force_generic == 3)) return launch_fused_x2(M, logd, fa, h_dm, nunits, st, launches);
+    const bool fast = fast_ok && force_generic != 1;
     cudaError_t e = cudaErrorInvalidValue;
     if (fast) {
         switch (M) {

@@ -1,0 +1,95 @@
+// cdmt_fused_common.cuh -- argument blocks and small device helpers shared by the fused per-DM
+// kernels (cdmt_fused.cu: scalar kernels; cdmt_fused2.cu: packed-FP32 + TMEM kernel).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace cdmt {
+
+template <bool ACCURATE>
+__device__ __forceinline__ float2 unit_phasor(float frac_cycles)
+{
+    float s, c;
+    if (ACCURATE) {
+        sincospif(2.0f * frac_cycles, &s, &c);
+    } else {
+        const float x = frac_cycles * 6.283185307179586f;
+        s = __sinf(x);
+        c = __cosf(x);
+    }
+    return make_float2(c, s);
+}
+
+__device__ __forceinline__ float2 unit_phasor_rt(float frac_cycles, int accurate)
+{
+    return accurate ? unit_phasor<true>(frac_cycles) : unit_phasor<false>(frac_cycles);
+}
+
+// fractional part in [-0.5, 0.5] of dm * g, exact to fp64 rounding
+__device__ __forceinline__ float frac_cycles(double dm, double g)
+{
+    const double magic = 6755399441055744.0;  // 1.5 * 2^52: adding it rounds to the nearest integer
+    const double n = fma(dm, g, magic) - magic;
+    return (float)fma(dm, g, -n);
+}
+
+constexpr int DM_PARAM_MAX = 1024;  // DM trials carried in the kernel parameter block (constant bank)
+
+struct DmParams {
+    double dm[DM_PARAM_MAX];
+};
+
+struct FusedArgs {
+    const float2 *spec;      // [units][2][nfft] swapped-halves spectra of this chunk
+    const float2 *tw;        // pass twiddles of the length-M backward transform
+    const double *dmlist;
+    const double *fcen;
+    float *out;
+    long long out_stride_dm;
+    int unit0, nsub, nchan, nfft, hdisc, ndec, vdec, ndm, dm_tile, chirp_ref, accurate;
+    int dm_first, dm_param0;  // DM range [dm_first, ndm) of this launch; dmp.dm[0] is trial dm_param0
+    double bw_mhz;
+    float scale;
+};
+
+// frequency set-up shared by both kernels: nu_0 of Eq. 1 and the offset of bin m (MHz)
+__device__ __forceinline__ void chirp_axes(const FusedArgs &a, int s, int c, int M, double *f0, double *f_bin0,
+                                           double *df)
+{
+    const double fc = a.fcen[s];
+    *df = a.bw_mhz / (double)a.nfft;
+    if (a.chirp_ref == 0) {
+        *f0 = fc + ((double)c + 0.5 - 0.5 * (double)a.nchan) * a.bw_mhz / (double)a.nchan;
+        *f_bin0 = -(double)(M / 2) * *df;
+    } else {
+        *f0 = fc;
+        *f_bin0 = (double)(c * M - a.nfft / 2) * *df;
+    }
+}
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(
+                     (unsigned)__cvta_generic_to_shared(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tWAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}" ::"r"((unsigned)__cvta_generic_to_shared(bar)),
+        "r"(parity)
+        : "memory");
+}
+
+// cdmt_fused2.cu
+bool fused_x2_supported(int M, int ndec, int hdisc);
+cudaError_t launch_fused_x2(int M, int logd, const FusedArgs &fa, const double *h_dm, int nunits, cudaStream_t st,
+                            long long *launches);
+
+}  // namespace cdmt
