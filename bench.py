@@ -198,6 +198,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--chunk-units", type=int, default=0)
     ap.add_argument("--dm-tile", type=int, default=0)
+    ap.add_argument("--fused-kernel", type=int, default=0, help="CDMT_OPT_FUSED_KERNEL (0 = library default)")
     ap.add_argument("--gen-threads", type=int, default=0)
     args = ap.parse_args()
 
@@ -258,6 +259,8 @@ def main():
         cdmt.cdmt_plan_set_option(plan, cdmt.OPT_CHUNK_UNITS, args.chunk_units)
     if args.dm_tile:
         cdmt.cdmt_plan_set_option(plan, cdmt.OPT_DM_TILE, args.dm_tile)
+    if args.fused_kernel:
+        cdmt.cdmt_plan_set_option(plan, cdmt.OPT_FUSED_KERNEL, args.fused_kernel)
     q = cdmt.cdmt_plan_query(plan, cfg.nsamp)
     nch = cfg.nsub * cfg.nchan
     nt = q["nout_per_chan"]

@@ -60,8 +60,10 @@ enum {
     CDMT_OPT_ACCURATE_SINCOS = 2, /* 1: sincospif instead of the fast approximation */
     CDMT_OPT_PROFILE = 3,     /* 1: record CUDA events round each kernel class (cdmt_profile_read) */
     CDMT_OPT_FUSED_KERNEL = 4, /* fused per-DM kernel: 0 = best applicable (default), 1 = general kernel (any ndec /
-                                  overlap), 2 = scalar fast kernel, 3 = packed-FP32 + tensor-memory kernel;
-                                  2 and 3 make cdmt_execute fail with CDMT_ERR_CUDA where they do not apply */
+                                  overlap), 2 = scalar fast kernel, 3 = packed-FP32 + tensor-memory kernel with the
+                                  even/odd half transforms in the register lanes, 4 = the same with the two
+                                  polarisations in the lanes (16 warps per SM); 2, 3 and 4 make cdmt_execute fail
+                                  with CDMT_ERR_CUDA where they do not apply */
     CDMT_OPT_FORCE_GENERIC = 4 /* older name of the same key (value 1) */
 };
 

@@ -19,7 +19,7 @@ OK, ERR_ARG, ERR_SIZE, ERR_WORKSPACE, ERR_CUDA, ERR_ALLOC = range(6)
 IN_CF32, IN_CI8 = 0, 1
 REF_CHANNEL, REF_SUBBAND = 0, 1
 OPT_CHUNK_UNITS, OPT_DM_TILE, OPT_ACCURATE_SINCOS, OPT_PROFILE, OPT_FORCE_GENERIC = 0, 1, 2, 3, 4
-OPT_FUSED_KERNEL = 4  # 0 auto, 1 general, 2 scalar fast, 3 packed-FP32 + TMEM
+OPT_FUSED_KERNEL = 4  # 0 auto, 1 general, 2 scalar fast, 3 packed half transforms + TMEM, 4 packed polarisations + TMEM
 
 EXPORTS = [
     "cdmt_plan_create", "cdmt_plan_destroy", "cdmt_plan_set_option", "cdmt_plan_query",

@@ -18,7 +18,7 @@ struct cdmt_plan {
     int dm_tile;             // 0 = all
     int accurate;
     int profile;             // record CUDA events around each kernel class
-    int force_generic;       // CDMT_OPT_FUSED_KERNEL: 0 auto, 1 generic, 2 scalar fast, 3 packed
+    int force_generic;       // CDMT_OPT_FUSED_KERNEL: 0 auto, 1 generic, 2 scalar fast, 3 packed halves, 4 packed pols
     long long last_launches;
     std::vector<cudaEvent_t> ev_pool;   // created lazily, reused
     size_t ev_used;
@@ -155,7 +155,7 @@ extern "C" int cdmt_plan_set_option(cdmt_plan *plan, int key, long long value)
         plan->profile = (int)value;
         return CDMT_OK;
     case CDMT_OPT_FUSED_KERNEL:
-        if (value < 0 || value > 3) return CDMT_ERR_ARG;
+        if (value < 0 || value > 4) return CDMT_ERR_ARG;
         plan->force_generic = (int)value;
         return CDMT_OK;
     default: return CDMT_ERR_ARG;

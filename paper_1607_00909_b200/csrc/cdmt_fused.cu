@@ -207,25 +207,6 @@ __device__ __forceinline__ void inplace_tail(float2 *v, float2 *ex, const float2
     }
 }
 
-// reduce-scatter over 2^LOGD adjacent lanes: in[n], n < 16, becomes out[j] = sum over the lane
-// group of slot n = (lane & (D-1)) + D j
-template <int LOGD, int S = 0>
-__device__ __forceinline__ void lane_reduce_scatter(float *a, int lane)
-{
-    if constexpr (S < LOGD) {
-        constexpr int cnt = 16 >> S;  // values held before this stage
-        const bool up = (lane >> S) & 1;
-#pragma unroll
-        for (int j = 0; j < cnt / 2; ++j) {
-            const float lo = a[2 * j], hi = a[2 * j + 1];
-            const float send = up ? lo : hi;
-            const float keep = up ? hi : lo;
-            a[j] = keep + __shfl_xor_sync(0xffffffffu, send, 1 << S);
-        }
-        lane_reduce_scatter<LOGD, S + 1>(a, lane);
-    }
-}
-
 template <int M, int LOGD>
 __global__ void __launch_bounds__(M / 16, (512 / (M / 16) > 16 ? 16 : (512 / (M / 16) < 1 ? 1 : 512 / (M / 16))))
 k_fused_fast(const FusedArgs a, const __grid_constant__ DmParams dmp)
@@ -426,12 +407,15 @@ cudaError_t launch_fused(const Geometry &g, const Workspace &ws, const float2 *s
     fa.dm_param0 = 0;
     int logd = 0;
     while ((1 << logd) < D) ++logd;
-    // force_generic carries CDMT_OPT_FUSED_KERNEL: 0 auto, 1 generic, 2 scalar fast, 3 packed (x2)
+    // force_generic carries CDMT_OPT_FUSED_KERNEL: 0 auto, 1 generic, 2 scalar fast, 3 packed halves (x2), 4 packed pols (pp)
     const bool fast_ok = !accurate && M >= 512 && D <= 32 && (1 << logd) == D && (g.hdisc % D) == 0 &&
                          poly_phase_ok(g, h_dm, h_fcen);
     const bool x2_ok = fast_ok && fused_x2_supported(M, D, g.hdisc);
+    const bool pp_ok = fast_ok && fused_pp_supported(M, D, g.hdisc);
+    if (force_generic == 4 && !pp_ok) return cudaErrorInvalidValue;
     if (force_generic == 3 && !x2_ok) return cudaErrorInvalidValue;
     if (force_generic == 2 && !fast_ok) return cudaErrorInvalidValue;
+    if (pp_ok && (force_generic == 0 || force_generic == 4)) return launch_fused_pp(M, logd, fa, h_dm, nunits, st, launches);
     if (x2_ok && (force_generic == 0 || force_generic == 3)) return launch_fused_x2(M, logd, fa, h_dm, nunits, st, launches);
     const bool fast = fast_ok && force_generic != 1;
     cudaError_t e = cudaErrorInvalidValue;

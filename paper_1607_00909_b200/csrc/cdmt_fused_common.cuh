@@ -87,9 +87,32 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity)
         : "memory");
 }
 
+// reduce-scatter over 2^LOGD adjacent lanes: in[n], n < 16, becomes out[j] = sum over the lane
+// group of slot n = (lane & (D-1)) + D j
+template <int LOGD, int S = 0>
+__device__ __forceinline__ void lane_reduce_scatter(float *a, int lane)
+{
+    if constexpr (S < LOGD) {
+        constexpr int cnt = 16 >> S;  // values held before this stage
+        const bool up = (lane >> S) & 1;
+#pragma unroll
+        for (int j = 0; j < cnt / 2; ++j) {
+            const float lo = a[2 * j], hi = a[2 * j + 1];
+            const float send = up ? lo : hi;
+            const float keep = up ? hi : lo;
+            a[j] = keep + __shfl_xor_sync(0xffffffffu, send, 1 << S);
+        }
+        lane_reduce_scatter<LOGD, S + 1>(a, lane);
+    }
+}
+
 // cdmt_fused2.cu
 bool fused_x2_supported(int M, int ndec, int hdisc);
 cudaError_t launch_fused_x2(int M, int logd, const FusedArgs &fa, const double *h_dm, int nunits, cudaStream_t st,
+                            long long *launches);
+// cdmt_fused3.cu
+bool fused_pp_supported(int M, int ndec, int hdisc);
+cudaError_t launch_fused_pp(int M, int logd, const FusedArgs &fa, const double *h_dm, int nunits, cudaStream_t st,
                             long long *launches);
 
 }  // namespace cdmt

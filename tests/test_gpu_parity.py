@@ -132,33 +132,42 @@ X2_SHAPES = [
     (2, 2 ** 15, 16384, 4096, 8, 8),      # 2048
     (1, 2 ** 16, 32768, 8192, 16, 32),    # 2048, ndec = 32
     (1, 2 ** 17, 65536, 32768, 16, 8),    # 4096, half of every block discarded
+    (1, 2 ** 17, 65536, 16384, 16, 1),    # 4096, no integration (kernel 4 only among the packed ones)
+    (1, 2 ** 16, 32768, 8192, 16, 4),     # 2048, ndec = 4
 ]
 
 
 @pytest.mark.parametrize("shape", X2_SHAPES)
 @pytest.mark.parametrize("ref", [synth.REF_CHANNEL, synth.REF_SUBBAND])
 def test_fused_kernel_variants(cdmt, shape, ref):
-    """CDMT_OPT_FUSED_KERNEL: packed-FP32 + TMEM (3), scalar fast (2) and general (1) kernels."""
+    """CDMT_OPT_FUSED_KERNEL: packed polarisations (4), packed half transforms (3), scalar fast (2)
+    and general (1) kernels."""
     nsub, nsamp, nfft, noverlap, nchan, ndec = shape
     cfg = synth.small_config(nsub=nsub, nsamp=nsamp, nfft=nfft, noverlap=noverlap, nchan=nchan,
                              ndec=ndec, dm=(0.0, 1.5, -3.5, 41.25, 96.0), f_lo=121.0)
     x = synth.generate(cfg, chirp_ref=ref)
     want = orc.run(orc.Params(**cfg.plan_kwargs(ref)), x)
-    for kern in (3, 2, 1):
+    M = nfft // nchan
+    kerns = [2, 1]
+    if ndec >= 8:
+        kerns.insert(0, 3)
+    if M <= 4096:
+        kerns.insert(0, 4)
+    for kern in kerns:
         got, _ = gpu_run(cdmt, cfg, x, ref, opts={cdmt.OPT_FUSED_KERNEL: kern})
         worst = check_filterbank(got, want)
         assert worst < TOL, (kern, worst)
     # a DM tile that does not divide ndm, one unit per chunk
-    got, _ = gpu_run(cdmt, cfg, x, ref, opts={cdmt.OPT_FUSED_KERNEL: 3, cdmt.OPT_DM_TILE: 2,
+    got, _ = gpu_run(cdmt, cfg, x, ref, opts={cdmt.OPT_FUSED_KERNEL: kerns[0], cdmt.OPT_DM_TILE: 2,
                                              cdmt.OPT_CHUNK_UNITS: 1})
     check_filterbank(got, want)
 
 
 def test_fused_kernel_choice_is_checked(cdmt):
-    """Kernels 2 and 3 refuse shapes they do not cover (status, not a wrong answer)."""
+    """Kernels 2, 3 and 4 refuse shapes they do not cover (status, not a wrong answer)."""
     cfg = synth.small_config(nsub=1, nsamp=2 ** 13, nfft=4096, noverlap=992, nchan=8, ndec=4, dm=(0.0, 3.0))
     x = synth.generate(cfg)
-    for kern in (2, 3):
+    for kern in (2, 3, 4):
         with pytest.raises(cdmt.CdmtError) as e:
             gpu_run(cdmt, cfg, x, opts={cdmt.OPT_FUSED_KERNEL: kern})
         assert e.value.status == cdmt.ERR_CUDA
