@@ -64,7 +64,8 @@ enum {
                                   even/odd half transforms in the register lanes, 4 = the same with the two
                                   polarisations in the lanes (16 warps per SM); 2, 3 and 4 make cdmt_execute fail
                                   with CDMT_ERR_CUDA where they do not apply */
-    CDMT_OPT_FORCE_GENERIC = 4 /* older name of the same key (value 1) */
+    CDMT_OPT_FORCE_GENERIC = 4, /* older name of the same key (value 1) */
+    CDMT_OPT_HOST_GROUP_BLOCKS = 5 /* cdmt_execute_host: blocks staged per group (0 = about 512 MiB of output) */
 };
 
 /*
@@ -130,13 +131,20 @@ int cdmt_execute(cdmt_plan *plan, const void *d_in, long long nsamp, long long i
  * copy to host).  h_in / h_out have the layouts of d_in / d_out (h_out planes dense:
  * stride nblock*Vd*nsub*nchan) and should be pinned for full copy speed.  The caller lends
  * device scratch `d_scratch` of at least cdmt_host_scratch_bytes(); input, workspace and
- * output are staged there in groups of blocks.  Copies and kernels are issued on
- * `cuda_stream`; the call returns after the last device-to-host copy has completed.
+ * output are staged there in groups of blocks, input and output double-buffered
+ * (the transfers, not the kernels, are the paper's bottleneck).  Kernels run on
+ * `cuda_stream`; the host-to-device copy of the next group and the device-to-host copy of the
+ * previous one run meanwhile on two streams the plan creates on first use (ordered after the
+ * work already queued on `cuda_stream`).  The call returns after the last device-to-host copy
+ * has completed; on error all three streams are drained before it returns.
  */
 int cdmt_execute_host(cdmt_plan *plan, const void *h_in, long long nsamp,
                       long long in_stride_pol, float *h_out, void *d_scratch,
                       size_t scratch_bytes, void *cuda_stream);
 int cdmt_host_scratch_bytes(const cdmt_plan *plan, long long nsamp, size_t *scratch_bytes);
+/* Bytes one cdmt_execute_host call copies host-to-device (each group re-sends the noverlap
+ * samples it shares with the previous one) and device-to-host.  Host arithmetic. */
+int cdmt_host_traffic_bytes(const cdmt_plan *plan, long long nsamp, size_t *h2d_bytes, size_t *d2h_bytes);
 
 /*
  * Stage entry points (used by the per-kernel parity tests; same validation rules).

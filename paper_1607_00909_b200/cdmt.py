@@ -19,11 +19,12 @@ OK, ERR_ARG, ERR_SIZE, ERR_WORKSPACE, ERR_CUDA, ERR_ALLOC = range(6)
 IN_CF32, IN_CI8 = 0, 1
 REF_CHANNEL, REF_SUBBAND = 0, 1
 OPT_CHUNK_UNITS, OPT_DM_TILE, OPT_ACCURATE_SINCOS, OPT_PROFILE, OPT_FORCE_GENERIC = 0, 1, 2, 3, 4
+OPT_HOST_GROUP_BLOCKS = 5
 OPT_FUSED_KERNEL = 4  # 0 auto, 1 general, 2 scalar fast, 3 packed half transforms + TMEM, 4 packed polarisations + TMEM
 
 EXPORTS = [
     "cdmt_plan_create", "cdmt_plan_destroy", "cdmt_plan_set_option", "cdmt_plan_query",
-    "cdmt_execute", "cdmt_execute_host", "cdmt_host_scratch_bytes", "cdmt_unpack",
+    "cdmt_execute", "cdmt_execute_host", "cdmt_host_scratch_bytes", "cdmt_host_traffic_bytes", "cdmt_unpack",
     "cdmt_forward_spectrum", "cdmt_sweep_seconds", "cdmt_min_overlap",
     "cdmt_measure_fp32_peak", "cdmt_last_launch_count", "cdmt_profile_read", "cdmt_strerror",
     "cdmt_version",
@@ -46,6 +47,7 @@ _lib.cdmt_plan_query.argtypes = [_vp, _ll, C.POINTER(_i), C.POINTER(_ll), C.POIN
 _lib.cdmt_execute.argtypes = [_vp, _vp, _ll, _ll, _vp, _ll, _vp, _sz, _vp]
 _lib.cdmt_execute_host.argtypes = [_vp, _vp, _ll, _ll, _vp, _vp, _sz, _vp]
 _lib.cdmt_host_scratch_bytes.argtypes = [_vp, _ll, C.POINTER(_sz)]
+_lib.cdmt_host_traffic_bytes.argtypes = [_vp, _ll, C.POINTER(_sz), C.POINTER(_sz)]
 _lib.cdmt_unpack.argtypes = [_vp, _vp, _ll, _ll, _vp, _vp]
 _lib.cdmt_forward_spectrum.argtypes = [_vp, _vp, _ll, _ll, _vp, _vp, _sz, _vp]
 _lib.cdmt_sweep_seconds.argtypes = [_d, _d, _d]
@@ -161,6 +163,12 @@ def cdmt_host_scratch_bytes(plan: Plan, nsamp: int) -> int:
     n = _sz()
     _check(_lib.cdmt_host_scratch_bytes(plan.handle, int(nsamp), C.byref(n)), "cdmt_host_scratch_bytes")
     return n.value
+
+
+def cdmt_host_traffic_bytes(plan: Plan, nsamp: int):
+    a, b = _sz(), _sz()
+    _check(_lib.cdmt_host_traffic_bytes(plan.handle, int(nsamp), C.byref(a), C.byref(b)), "cdmt_host_traffic_bytes")
+    return a.value, b.value
 
 
 def cdmt_execute_host(plan: Plan, h_in, nsamp: int, in_stride_pol: int, h_out, d_scratch,

@@ -18,13 +18,33 @@ struct cdmt_plan {
     int dm_tile;             // 0 = all
     int accurate;
     int profile;             // record CUDA events around each kernel class
+    long long host_group;    // CDMT_OPT_HOST_GROUP_BLOCKS: blocks per staged group of the host path (0 = automatic)
     int force_generic;       // CDMT_OPT_FUSED_KERNEL: 0 auto, 1 generic, 2 scalar fast, 3 packed halves, 4 packed pols
     long long last_launches;
     std::vector<cudaEvent_t> ev_pool;   // created lazily, reused
     size_t ev_used;
     struct Span { size_t e0, e1; int kind; };   // kind 0: forward FFT passes, 1: fused per-DM kernel
     std::vector<Span> spans;
+    // host-buffer path (cdmt_execute_host): copy streams and the events that order the double buffers
+    cudaStream_t s_in, s_out;
+    cudaEvent_t ev_start, ev_h2d[2], ev_comp[2], ev_d2h[2];
+    bool host_ready;
 };
+
+// Lazily create the copy streams and ordering events of the host-buffer path.
+static bool plan_host_pipeline(cdmt_plan *p)
+{
+    if (p->host_ready) return true;
+    bool ok = cudaStreamCreateWithFlags(&p->s_in, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaStreamCreateWithFlags(&p->s_out, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaEventCreateWithFlags(&p->ev_start, cudaEventDisableTiming) == cudaSuccess;
+    for (int i = 0; i < 2 && ok; ++i)
+        ok = cudaEventCreateWithFlags(&p->ev_h2d[i], cudaEventDisableTiming) == cudaSuccess &&
+             cudaEventCreateWithFlags(&p->ev_comp[i], cudaEventDisableTiming) == cudaSuccess &&
+             cudaEventCreateWithFlags(&p->ev_d2h[i], cudaEventDisableTiming) == cudaSuccess;
+    p->host_ready = ok;
+    return ok;
+}
 
 static cudaEvent_t plan_event(cdmt_plan *p, size_t *idx)
 {
@@ -122,6 +142,9 @@ extern "C" int cdmt_plan_create(cdmt_plan **plan, int nsub, const double *fcen_m
     p->force_generic = 0;
     p->ev_used = 0;
     p->last_launches = 0;
+    p->host_ready = false;
+    p->host_group = 0;
+    p->s_in = p->s_out = nullptr;
     *plan = p;
     return CDMT_OK;
 }
@@ -130,6 +153,16 @@ extern "C" int cdmt_plan_destroy(cdmt_plan *plan)
 {
     if (!plan) return CDMT_ERR_ARG;
     for (cudaEvent_t e : plan->ev_pool) cudaEventDestroy(e);
+    if (plan->host_ready) {
+        cudaStreamDestroy(plan->s_in);
+        cudaStreamDestroy(plan->s_out);
+        cudaEventDestroy(plan->ev_start);
+        for (int i = 0; i < 2; ++i) {
+            cudaEventDestroy(plan->ev_h2d[i]);
+            cudaEventDestroy(plan->ev_comp[i]);
+            cudaEventDestroy(plan->ev_d2h[i]);
+        }
+    }
     delete plan;
     return CDMT_OK;
 }
@@ -157,6 +190,10 @@ extern "C" int cdmt_plan_set_option(cdmt_plan *plan, int key, long long value)
     case CDMT_OPT_FUSED_KERNEL:
         if (value < 0 || value > 4) return CDMT_ERR_ARG;
         plan->force_generic = (int)value;
+        return CDMT_OK;
+    case CDMT_OPT_HOST_GROUP_BLOCKS:
+        if (value < 0 || value > (1LL << 30)) return CDMT_ERR_ARG;
+        plan->host_group = value;
         return CDMT_OK;
     default: return CDMT_ERR_ARG;
     }
@@ -332,19 +369,25 @@ extern "C" int cdmt_unpack(cdmt_plan *plan, const void *d_in, long long nsamp, l
 }
 
 // ---- host-buffer path --------------------------------------------------------------------
-// blocks per staged group: keep the staged output near 1 GiB
+// the observation is streamed through the GPU in groups of
+// blocks, and the paper's measured bottleneck is this traffic, not the kernels.  Input and
+// output staging buffers are doubled: the host-to-device copy of group i+1 and the
+// device-to-host copy of group i-1 run on their own streams while group i computes.
+
+// blocks per staged group: keep the staged output near 512 MiB
 static long long host_group_blocks(const cdmt_plan *plan, long long nb)
 {
     const Geometry &g = plan->g;
     const long long per_block = (long long)g.ndm * g.vdec * g.nsub * g.nchan * (long long)sizeof(float);
-    long long gb = (1LL << 30) / (per_block > 0 ? per_block : 1);
+    long long gb = (1LL << 29) / (per_block > 0 ? per_block : 1);
+    if (plan->host_group > 0) gb = plan->host_group;
     if (gb < 1) gb = 1;
     if (gb > nb) gb = nb;
     return gb;
 }
 
 struct HostLayout {
-    size_t in_off, in_bytes, ws_off, ws_bytes, out_off, out_bytes, total;
+    size_t in_off[2], in_bytes, ws_off, ws_bytes, out_off[2], out_bytes, total;
     long long gb, in_rowlen;
 };
 
@@ -359,14 +402,17 @@ static int host_layout(const cdmt_plan *plan, long long nsamp, HostLayout *L)
     rowlen = (rowlen + 7) & ~7LL;  // keep rows 16-byte aligned for both word sizes
     L->in_rowlen = rowlen;
     auto al = [](size_t x) { return (x + 255) & ~(size_t)255; };
-    L->in_off = 0;
+    const int nbuf = L->gb < nb ? 2 : 1;  // a single group needs no second buffer
     L->in_bytes = al((size_t)rowlen * esz * 2 * g.nsub);
-    L->ws_off = L->in_off + L->in_bytes;
+    L->in_off[0] = 0;
+    L->in_off[1] = nbuf == 2 ? L->in_bytes : 0;
+    L->ws_off = L->in_bytes * nbuf;
     const long long cu = chunk_units_for(plan, L->gb * g.nsub);
     L->ws_bytes = al(workspace_layout(g, (int)cu, nullptr, nullptr));
-    L->out_off = L->ws_off + L->ws_bytes;
     L->out_bytes = al((size_t)g.ndm * L->gb * g.vdec * g.nsub * g.nchan * sizeof(float));
-    L->total = L->out_off + L->out_bytes;
+    L->out_off[0] = L->ws_off + L->ws_bytes;
+    L->out_off[1] = nbuf == 2 ? L->out_off[0] + L->out_bytes : L->out_off[0];
+    L->total = L->out_off[0] + L->out_bytes * nbuf;
     return CDMT_OK;
 }
 
@@ -377,6 +423,26 @@ extern "C" int cdmt_host_scratch_bytes(const cdmt_plan *plan, long long nsamp, s
     int rc = host_layout(plan, nsamp, &L);
     if (rc) return rc;
     *scratch_bytes = L.total;
+    return CDMT_OK;
+}
+
+// Bytes one cdmt_execute_host call moves over the host link (the overlap between groups is re-sent).
+extern "C" int cdmt_host_traffic_bytes(const cdmt_plan *plan, long long nsamp, size_t *h2d_bytes, size_t *d2h_bytes)
+{
+    if (!plan) return CDMT_ERR_ARG;
+    HostLayout L;
+    int rc = host_layout(plan, nsamp, &L);
+    if (rc) return rc;
+    const Geometry &g = plan->g;
+    const long long nb = nblock_for(g, nsamp);
+    const size_t esz = g.in_dtype == CDMT_IN_CI8 ? 2 : 8;
+    size_t in = 0;
+    for (long long b0 = 0; b0 < nb; b0 += L.gb) {
+        const long long nbg = (nb - b0 < L.gb) ? nb - b0 : L.gb;
+        in += (size_t)((nbg - 1) * g.step + g.nfft) * esz * 2 * g.nsub;
+    }
+    if (h2d_bytes) *h2d_bytes = in;
+    if (d2h_bytes) *d2h_bytes = (size_t)g.ndm * (size_t)(nb * g.vdec) * (size_t)g.nsub * g.nchan * sizeof(float);
     return CDMT_OK;
 }
 
@@ -391,35 +457,75 @@ extern "C" int cdmt_execute_host(cdmt_plan *plan, const void *h_in, long long ns
     int rc = host_layout(plan, nsamp, &L);
     if (rc) return rc;
     if (scratch_bytes < L.total) return CDMT_ERR_WORKSPACE;
+    if (!plan_host_pipeline(plan)) return check_cuda(cudaErrorUnknown);
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const long long nb = nblock_for(g, nsamp);
     const long long esz = g.in_dtype == CDMT_IN_CI8 ? 2 : 8;
     char *base = reinterpret_cast<char *>(d_scratch);
-    char *d_in = base + L.in_off;
-    float *d_out = reinterpret_cast<float *>(base + L.out_off);
     const size_t nchtot = (size_t)g.nsub * g.nchan;
     const size_t plane_host = (size_t)nb * g.vdec * nchtot;
+    const long long ngroup = (nb + L.gb - 1) / L.gb;
     long long launches = 0;
-    for (long long b0 = 0; b0 < nb; b0 += L.gb) {
+
+    // the copy streams start after whatever the caller queued on `st` before this call
+    rc = check_cuda(cudaEventRecord(plan->ev_start, st));
+    if (!rc) rc = check_cuda(cudaStreamWaitEvent(plan->s_in, plan->ev_start, 0));
+    if (!rc) rc = check_cuda(cudaStreamWaitEvent(plan->s_out, plan->ev_start, 0));
+
+    auto h2d = [&](long long i) -> int {
+        const int k = (int)(i & 1);
+        const long long b0 = i * L.gb;
         const long long nbg = (nb - b0 < L.gb) ? nb - b0 : L.gb;
         const long long len = (nbg - 1) * g.step + g.nfft;
-        rc = check_cuda(cudaMemcpy2DAsync(d_in, (size_t)L.in_rowlen * esz,
-                                          reinterpret_cast<const char *>(h_in) + (size_t)b0 * g.step * esz,
-                                          (size_t)in_stride_pol * esz, (size_t)len * esz, (size_t)2 * g.nsub,
-                                          cudaMemcpyHostToDevice, st));
-        if (rc) return rc;
+        // buffer k was last read by the kernels of group i-2
+        if (i >= 2) {
+            int r = check_cuda(cudaStreamWaitEvent(plan->s_in, plan->ev_comp[k], 0));
+            if (r) return r;
+        }
+        int r = check_cuda(cudaMemcpy2DAsync(base + L.in_off[k], (size_t)L.in_rowlen * esz,
+                                             reinterpret_cast<const char *>(h_in) + (size_t)b0 * g.step * esz,
+                                             (size_t)in_stride_pol * esz, (size_t)len * esz, (size_t)2 * g.nsub,
+                                             cudaMemcpyHostToDevice, plan->s_in));
+        if (r) return r;
+        return check_cuda(cudaEventRecord(plan->ev_h2d[k], plan->s_in));
+    };
+
+    if (!rc) rc = h2d(0);
+    for (long long i = 0; i < ngroup && !rc; ++i) {
+        const int k = (int)(i & 1);
+        const long long b0 = i * L.gb;
+        const long long nbg = (nb - b0 < L.gb) ? nb - b0 : L.gb;
         const size_t plane_dev = (size_t)nbg * g.vdec * nchtot;
-        rc = run_chunks(plan, d_in, L.in_rowlen, nbg, d_out, (long long)plane_dev, nullptr, base + L.ws_off,
-                        L.ws_bytes, st);
-        if (rc) return rc;
+        float *d_out = reinterpret_cast<float *>(base + L.out_off[k]);
+        // compute of group i: needs its input, and output buffer k drained by the copy of group i-2
+        rc = check_cuda(cudaStreamWaitEvent(st, plan->ev_h2d[k], 0));
+        if (!rc && i >= 2) rc = check_cuda(cudaStreamWaitEvent(st, plan->ev_d2h[k], 0));
+        if (rc) break;
+        rc = run_chunks(plan, base + L.in_off[k], L.in_rowlen, nbg, d_out, (long long)plane_dev, nullptr,
+                        base + L.ws_off, L.ws_bytes, st);
+        if (rc) break;
         launches += plan->last_launches;
-        rc = check_cuda(cudaMemcpy2DAsync(h_out + (size_t)b0 * g.vdec * nchtot, plane_host * sizeof(float), d_out,
-                                          plane_dev * sizeof(float), plane_dev * sizeof(float), (size_t)g.ndm,
-                                          cudaMemcpyDeviceToHost, st));
-        if (rc) return rc;
+        rc = check_cuda(cudaEventRecord(plan->ev_comp[k], st));
+        if (rc) break;
+        // the next group's input travels while this group computes
+        if (i + 1 < ngroup) {
+            rc = h2d(i + 1);
+            if (rc) break;
+        }
+        rc = check_cuda(cudaStreamWaitEvent(plan->s_out, plan->ev_comp[k], 0));
+        if (!rc)
+            rc = check_cuda(cudaMemcpy2DAsync(h_out + (size_t)b0 * g.vdec * nchtot, plane_host * sizeof(float), d_out,
+                                              plane_dev * sizeof(float), plane_dev * sizeof(float), (size_t)g.ndm,
+                                              cudaMemcpyDeviceToHost, plan->s_out));
+        if (!rc) rc = check_cuda(cudaEventRecord(plan->ev_d2h[k], plan->s_out));
     }
     plan->last_launches = launches;
-    return check_cuda(cudaStreamSynchronize(st));
+    // drain all three streams whatever happened, so that the scratch can be reused or freed
+    const int r1 = check_cuda(cudaStreamSynchronize(plan->s_in));
+    const int r2 = check_cuda(cudaStreamSynchronize(st));
+    const int r3 = check_cuda(cudaStreamSynchronize(plan->s_out));
+    if (rc) return rc;
+    return r1 ? r1 : (r2 ? r2 : r3);
 }
 
 // n_d n_c >= r t_d for the lowest-frequency channel (or subband) at the largest |DM|.

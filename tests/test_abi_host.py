@@ -80,6 +80,27 @@ def test_chunk_option_changes_workspace_only(cdmt):
     assert q["nblock"] == 42
 
 
+def test_host_path_group_arithmetic(cdmt):
+    """cdmt_execute_host stages groups of blocks; the overlap between groups is re-sent."""
+    cfg = synth.make_config("c3")
+    plan = cdmt.cdmt_plan_create(**cfg.plan_kwargs())
+    esz, rows = 8, 2 * cfg.nsub
+    for gb in (1, 3, 5, 42):
+        cdmt.cdmt_plan_set_option(plan, cdmt.OPT_HOST_GROUP_BLOCKS, gb)
+        h2d, d2h = cdmt.cdmt_host_traffic_bytes(plan, cfg.nsamp)
+        want = 0
+        for b0 in range(0, 42, gb):
+            nbg = min(gb, 42 - b0)
+            want += ((nbg - 1) * cfg.step + cfg.nfft) * esz * rows
+        assert h2d == want
+        assert d2h == cdmt.cdmt_plan_query(plan, cfg.nsamp)["out_bytes"]
+        assert cdmt.cdmt_host_scratch_bytes(plan, cfg.nsamp) > 0
+    # one group: exactly the consumed samples once
+    assert h2d == cdmt.cdmt_plan_query(plan, cfg.nsamp)["nsamp_consumed"] * esz * rows
+    with pytest.raises(cdmt.CdmtError):
+        cdmt.cdmt_plan_set_option(plan, cdmt.OPT_HOST_GROUP_BLOCKS, -1)
+
+
 def bad(cdmt, status, **over):
     kw = dict(nsub=2, fcen_mhz=[150.0, 150.2], bw_mhz=synth.BW_MHZ, nfft=4096, noverlap=1024,
               nchan=8, ndec=4, dm=[0.0, 1.0])

@@ -255,6 +255,16 @@ def test_host_path_matches_device_path(cdmt):
     scratch = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
     cdmt.cdmt_execute_host(plan, h_in.data_ptr(), cfg.nsamp, cfg.nsamp, h_out.data_ptr(), scratch, nbytes)
     assert np.array_equal(h_out.numpy(), dev)
+    # double-buffered staging: 1, 2 and 3 blocks per group (10 blocks: odd/even groups, ragged last group)
+    assert cdmt.cdmt_plan_query(plan, cfg.nsamp)["nblock"] == 10
+    for gb in (1, 2, 3):
+        cdmt.cdmt_plan_set_option(plan, cdmt.OPT_HOST_GROUP_BLOCKS, gb)
+        nbytes = cdmt.cdmt_host_scratch_bytes(plan, cfg.nsamp)
+        scratch = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+        h_out.fill_(-1.0)
+        for _ in range(2):      # the second call reuses streams and events
+            cdmt.cdmt_execute_host(plan, h_in.data_ptr(), cfg.nsamp, cfg.nsamp, h_out.data_ptr(), scratch, nbytes)
+        assert np.array_equal(h_out.numpy(), dev), gb
 
 
 def test_errors_are_codes_not_crashes(cdmt):
