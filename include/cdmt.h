@@ -62,8 +62,9 @@ enum {
     CDMT_OPT_FUSED_KERNEL = 4, /* fused per-DM kernel: 0 = best applicable (default), 1 = general kernel (any ndec /
                                   overlap), 2 = scalar fast kernel, 3 = packed-FP32 + tensor-memory kernel with the
                                   even/odd half transforms in the register lanes, 4 = the same with the two
-                                  polarisations in the lanes (16 warps per SM); 2, 3 and 4 make cdmt_execute fail
-                                  with CDMT_ERR_CUDA where they do not apply */
+                                  polarisations in the lanes (16 warps per SM), 5 = kernel 4 software-pipelined
+                                  (chirp of the next trial formed in the shadow of the block barrier); 2 to 5
+                                  make cdmt_execute fail with CDMT_ERR_CUDA where they do not apply */
     CDMT_OPT_FORCE_GENERIC = 4, /* older name of the same key (value 1) */
     CDMT_OPT_HOST_GROUP_BLOCKS = 5 /* cdmt_execute_host: blocks staged per group (0 = about 512 MiB of output) */
 };

@@ -13,7 +13,8 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libcdmt.so")
+# CDMT_LIBRARY selects another build of the same library (e.g. one compiled with other flags)
+LIB_PATH = os.environ.get("CDMT_LIBRARY") or os.path.join(_HERE, "libcdmt.so")
 
 OK, ERR_ARG, ERR_SIZE, ERR_WORKSPACE, ERR_CUDA, ERR_ALLOC = range(6)
 IN_CF32, IN_CI8 = 0, 1

@@ -19,7 +19,7 @@ struct cdmt_plan {
     int accurate;
     int profile;             // record CUDA events around each kernel class
     long long host_group;    // CDMT_OPT_HOST_GROUP_BLOCKS: blocks per staged group of the host path (0 = automatic)
-    int force_generic;       // CDMT_OPT_FUSED_KERNEL: 0 auto, 1 generic, 2 scalar fast, 3 packed halves, 4 packed pols
+    int force_generic;       // CDMT_OPT_FUSED_KERNEL: 0 auto, 1 generic, 2 scalar fast, 3 packed halves, 4 packed pols, 5 pipelined
     long long last_launches;
     std::vector<cudaEvent_t> ev_pool;   // created lazily, reused
     size_t ev_used;
@@ -188,7 +188,7 @@ extern "C" int cdmt_plan_set_option(cdmt_plan *plan, int key, long long value)
         plan->profile = (int)value;
         return CDMT_OK;
     case CDMT_OPT_FUSED_KERNEL:
-        if (value < 0 || value > 4) return CDMT_ERR_ARG;
+        if (value < 0 || value > 5) return CDMT_ERR_ARG;
         plan->force_generic = (int)value;
         return CDMT_OK;
     case CDMT_OPT_HOST_GROUP_BLOCKS:

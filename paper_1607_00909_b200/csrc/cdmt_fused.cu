@@ -390,6 +390,17 @@ static bool poly_phase_ok(const Geometry &g, const double *h_dm, const double *h
     return P * x * x * x * x * x * x < 1e-7;
 }
 
+// Upper bound on |phase| of Eq. 1 in cycles over all bins, subbands and DM trials.
+static double phase_cycles_bound(const Geometry &g, const double *h_dm, const double *h_fcen)
+{
+    double dmax = 0.0, fmin = h_fcen[0];
+    for (int d = 0; d < g.ndm; ++d) dmax = fabs(h_dm[d]) > dmax ? fabs(h_dm[d]) : dmax;
+    for (int s = 0; s < g.nsub; ++s) fmin = h_fcen[s] < fmin ? h_fcen[s] : fmin;
+    const double flo = fmin - 0.5 * g.bw_mhz;
+    const double fmax = g.chirp_ref == 0 ? 0.5 * g.bw_mhz / g.nchan : 0.5 * g.bw_mhz;
+    return dmax * fmax * fmax / (2.41e-10 * flo * flo * flo);
+}
+
 cudaError_t launch_fused(const Geometry &g, const Workspace &ws, const float2 *spec, int unit0, int nunits,
                          float *d_out, long long out_stride_dm, int dm_tile, int accurate, int force_generic,
                          const double *h_dm, const double *h_fcen, cudaStream_t st, long long *launches)
@@ -407,11 +418,16 @@ cudaError_t launch_fused(const Geometry &g, const Workspace &ws, const float2 *s
     fa.dm_param0 = 0;
     int logd = 0;
     while ((1 << logd) < D) ++logd;
-    // force_generic carries CDMT_OPT_FUSED_KERNEL: 0 auto, 1 generic, 2 scalar fast, 3 packed halves (x2), 4 packed pols (pp)
+    // force_generic carries CDMT_OPT_FUSED_KERNEL: 0 auto, 1 generic, 2 scalar fast, 3 packed halves (x2),
+    // 4 packed pols (pp), 5 packed pols, software-pipelined chirp (sp)
     const bool fast_ok = !accurate && M >= 512 && D <= 32 && (1 << logd) == D && (g.hdisc % D) == 0 &&
                          poly_phase_ok(g, h_dm, h_fcen);
     const bool x2_ok = fast_ok && fused_x2_supported(M, D, g.hdisc);
     const bool pp_ok = fast_ok && fused_pp_supported(M, D, g.hdisc);
+    // sp reduces the phase mod 1 with a 2^20 magic number: |phase| must stay below 2^19 cycles
+    const bool sp_ok = fast_ok && fused_sp_supported(M, D, g.hdisc) && phase_cycles_bound(g, h_dm, h_fcen) < 262144.0;
+    if (force_generic == 5 && !sp_ok) return cudaErrorInvalidValue;
+    if (sp_ok && (force_generic == 0 || force_generic == 5)) return launch_fused_sp(M, logd, fa, h_dm, nunits, st, launches);
     if (force_generic == 4 && !pp_ok) return cudaErrorInvalidValue;
     if (force_generic == 3 && !x2_ok) return cudaErrorInvalidValue;
     if (force_generic == 2 && !fast_ok) return cudaErrorInvalidValue;

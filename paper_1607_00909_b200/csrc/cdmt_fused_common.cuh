@@ -115,4 +115,9 @@ bool fused_pp_supported(int M, int ndec, int hdisc);
 cudaError_t launch_fused_pp(int M, int logd, const FusedArgs &fa, const double *h_dm, int nunits, cudaStream_t st,
                             long long *launches);
 
+// cdmt_fused4.cu
+bool fused_sp_supported(int M, int ndec, int hdisc);
+cudaError_t launch_fused_sp(int M, int logd, const FusedArgs &fa, const double *h_dm, int nunits, cudaStream_t st,
+                            long long *launches);
+
 }  // namespace cdmt

@@ -140,8 +140,8 @@ X2_SHAPES = [
 @pytest.mark.parametrize("shape", X2_SHAPES)
 @pytest.mark.parametrize("ref", [synth.REF_CHANNEL, synth.REF_SUBBAND])
 def test_fused_kernel_variants(cdmt, shape, ref):
-    """CDMT_OPT_FUSED_KERNEL: packed polarisations (4), packed half transforms (3), scalar fast (2)
-    and general (1) kernels."""
+    """CDMT_OPT_FUSED_KERNEL: software-pipelined packed polarisations (5), packed polarisations (4),
+    packed half transforms (3), scalar fast (2) and general (1) kernels."""
     nsub, nsamp, nfft, noverlap, nchan, ndec = shape
     cfg = synth.small_config(nsub=nsub, nsamp=nsamp, nfft=nfft, noverlap=noverlap, nchan=nchan,
                              ndec=ndec, dm=(0.0, 1.5, -3.5, 41.25, 96.0), f_lo=121.0)
@@ -153,6 +153,7 @@ def test_fused_kernel_variants(cdmt, shape, ref):
         kerns.insert(0, 3)
     if M <= 4096:
         kerns.insert(0, 4)
+        kerns.insert(0, 5)
     for kern in kerns:
         got, _ = gpu_run(cdmt, cfg, x, ref, opts={cdmt.OPT_FUSED_KERNEL: kern})
         worst = check_filterbank(got, want)
@@ -164,10 +165,10 @@ def test_fused_kernel_variants(cdmt, shape, ref):
 
 
 def test_fused_kernel_choice_is_checked(cdmt):
-    """Kernels 2, 3 and 4 refuse shapes they do not cover (status, not a wrong answer)."""
+    """Kernels 2 to 5 refuse shapes they do not cover (status, not a wrong answer)."""
     cfg = synth.small_config(nsub=1, nsamp=2 ** 13, nfft=4096, noverlap=992, nchan=8, ndec=4, dm=(0.0, 3.0))
     x = synth.generate(cfg)
-    for kern in (2, 3, 4):
+    for kern in (2, 3, 4, 5):
         with pytest.raises(cdmt.CdmtError) as e:
             gpu_run(cdmt, cfg, x, opts={cdmt.OPT_FUSED_KERNEL: kern})
         assert e.value.status == cdmt.ERR_CUDA
