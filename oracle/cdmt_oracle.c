@@ -312,3 +312,99 @@ int oracle_channel_timeseries(const oracle_params *p, int s, int c, double dm, c
     free(Xs); free(H); free(Z); free(Zsw);
     return rc;
 }
+
+/* ------------------------------------------------------------------------------------------
+ * Redigitisation to 8 bit: Algorithm 1 l.104-106 ("compute block sums", "compute channel
+ * statistics", "redigitize").  Same four steps, same
+ * order, statistics in double.
+ *
+ *   fb      [ndm][nblock*vd][nch] float32 filterbank of ONE batch of nblock data blocks
+ *           (what oracle_run returns); statistics are per DM trial and per channel over the
+ *           nblock*vd samples of the batch ("the floating point timeseries of each
+ *           channel of N_FFT (M_bin - n_d) samples"; reading Q19)
+ *   segsum  [ndm][nblock][nch][2]: sum of I and of I^2 over the vd samples that block b gave to
+ *           the channel ("sums of intensity and intensity squared for segments of M samples";
+ *           reading Q20: one segment = one data block's samples)
+ *   mean, std [ndm][nch]: mean = sum I / n,  std = sqrt(max(0, sum I^2 / n - mean^2)),
+ *           n = nblock*vd ("average and standard deviation of each channel" from the segment
+ *           sums; population form, reading Q21)
+ *   offset, scale [ndm][nch] float32 and codes [ndm][nblock*vd][nch] uint8: the paper says only
+ *           that offset and scale follow from mean and std; reading Q22:
+ *               scale  = std / qstd          (1 if std == 0)
+ *               offset = mean - qmean * scale
+ *               code   = clip(rint((I - offset) / scale), 0, 255)
+ *           so that a channel's codes have mean qmean and standard deviation qstd.  offset and
+ *           scale are rounded to float32 once; the decision (subtract, divide, round half to
+ *           even, clip) is taken in float32, the precision of the paper's data path
+ *           (cufftComplex / float), one correctly rounded operation at a time.
+ * Any of segsum, mean, std, offset, scale, codes may be NULL.
+ */
+int oracle_redigitize(const float *fb, long ndm, long nblock, long vd, long nch, double qmean, double qstd,
+                      double *segsum, double *mean, double *std, float *offset, float *scale, uint8_t *codes)
+{
+    if (!fb || ndm < 1 || nblock < 1 || vd < 1 || nch < 1 || !(qstd > 0.0)) return 1;
+    const long nt = nblock * vd;
+    for (long d = 0; d < ndm; d++) {
+        const float *f = fb + (size_t)d * nt * nch;
+        for (long c = 0; c < nch; c++) {
+            /* compute block sums (l.104) */
+            double tot = 0.0, tot2 = 0.0;
+            for (long b = 0; b < nblock; b++) {
+                double s1 = 0.0, s2 = 0.0;
+                for (long q = 0; q < vd; q++) {
+                    const double v = (double)f[(size_t)(b * vd + q) * nch + c];
+                    s1 += v;
+                    s2 += v * v;
+                }
+                if (segsum) {
+                    segsum[(((size_t)d * nblock + b) * nch + c) * 2 + 0] = s1;
+                    segsum[(((size_t)d * nblock + b) * nch + c) * 2 + 1] = s2;
+                }
+                /* compute channel statistics (l.105): the segment sums are added up */
+                tot += s1;
+                tot2 += s2;
+            }
+            const double mu = tot / (double)nt;
+            double var = tot2 / (double)nt - mu * mu;
+            if (var < 0.0) var = 0.0;
+            const double sd = sqrt(var);
+            if (mean) mean[(size_t)d * nch + c] = mu;
+            if (std) std[(size_t)d * nch + c] = sd;
+            /* redigitize (l.106) */
+            const double sc64 = sd > 0.0 ? sd / qstd : 1.0;
+            const float sc = (float)sc64;
+            const float off = (float)(mu - qmean * sc64);
+            if (scale) scale[(size_t)d * nch + c] = sc;
+            if (offset) offset[(size_t)d * nch + c] = off;
+            if (codes)
+                for (long t = 0; t < nt; t++) {
+                    volatile float diff = f[(size_t)t * nch + c] - off; /* float32 subtraction */
+                    volatile float quot = diff / sc;                    /* float32 division */
+                    float r = nearbyintf(quot);                         /* round half to even */
+                    if (!(r >= 0.0f)) r = 0.0f;
+                    if (r > 255.0f) r = 255.0f;
+                    codes[((size_t)d * nt + t) * nch + c] = (uint8_t)r;
+                }
+        }
+    }
+    return 0;
+}
+
+/* The decision of l.106 alone, with offset and scale GIVEN (float32, [ndm][nch]): used to
+ * check a quantiser bit for bit on the offsets and scales it reports itself. */
+int oracle_quantize(const float *fb, long ndm, long nt, long nch, const float *offset, const float *scale,
+                    uint8_t *codes)
+{
+    if (!fb || !offset || !scale || !codes) return 1;
+    for (long d = 0; d < ndm; d++)
+        for (long t = 0; t < nt; t++)
+            for (long c = 0; c < nch; c++) {
+                volatile float diff = fb[((size_t)d * nt + t) * nch + c] - offset[(size_t)d * nch + c];
+                volatile float quot = diff / scale[(size_t)d * nch + c];
+                float r = nearbyintf(quot);
+                if (!(r >= 0.0f)) r = 0.0f;
+                if (r > 255.0f) r = 255.0f;
+                codes[((size_t)d * nt + t) * nch + c] = (uint8_t)r;
+            }
+    return 0;
+}

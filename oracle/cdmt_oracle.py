@@ -27,7 +27,7 @@ def build(force: bool = False) -> str:
     """Compile the oracle with gcc (plain -O2, no fast-math)."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         tmp = _LIB + ".tmp%d" % os.getpid()
-        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-o", tmp, _SRC, "-lm"])
+        subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", "-o", tmp, _SRC, "-lm"])
         os.replace(tmp, _LIB)
     return _LIB
 
@@ -63,6 +63,8 @@ def lib():
         L.oracle_run.argtypes = [C.POINTER(_Params), C.c_void_p, C.c_long, C.c_void_p, C.c_void_p]
         L.oracle_channel_timeseries.argtypes = [C.POINTER(_Params), C.c_int, C.c_int, C.c_double,
                                                 C.c_void_p, C.c_void_p]
+        L.oracle_redigitize.argtypes = [C.c_void_p] + [C.c_long] * 4 + [C.c_double] * 2 + [C.c_void_p] * 6
+        L.oracle_quantize.argtypes = [C.c_void_p] + [C.c_long] * 3 + [C.c_void_p] * 3
         _lib = L
     return _lib
 
@@ -178,3 +180,36 @@ def run(p: Params, x: np.ndarray, want64: bool = False):
     if rc:
         raise RuntimeError("oracle_run rc=%d" % rc)
     return (out, out64) if want64 else out
+
+
+QMEAN, QSTD = 64.0, 16.0   # reading Q22: code mean and standard deviation of a redigitised channel
+
+
+def redigitize(fb: np.ndarray, nblock: int, qmean: float = QMEAN, qstd: float = QSTD) -> dict:
+    """Alg. 1 l.104-106 on one batch: fb [ndm][nblock*vd][nch] float32 ->
+    dict(segsum [ndm][nblock][nch][2], mean, std [ndm][nch] float64, offset, scale float32, codes uint8)."""
+    fb = np.ascontiguousarray(fb, dtype=np.float32)
+    ndm, nt, nch = fb.shape
+    assert nt % nblock == 0
+    vd = nt // nblock
+    r = dict(segsum=np.empty((ndm, nblock, nch, 2)), mean=np.empty((ndm, nch)), std=np.empty((ndm, nch)),
+             offset=np.empty((ndm, nch), np.float32), scale=np.empty((ndm, nch), np.float32),
+             codes=np.empty((ndm, nt, nch), np.uint8))
+    rc = lib().oracle_redigitize(fb.ctypes.data, ndm, nblock, vd, nch, float(qmean), float(qstd),
+                                 *[r[k].ctypes.data for k in ("segsum", "mean", "std", "offset", "scale", "codes")])
+    if rc:
+        raise ValueError("oracle_redigitize rc=%d" % rc)
+    return r
+
+
+def quantize(fb: np.ndarray, offset: np.ndarray, scale: np.ndarray) -> np.ndarray:
+    """The float32 decision of l.106 with given per-(DM, channel) offset and scale."""
+    fb = np.ascontiguousarray(fb, dtype=np.float32)
+    ndm, nt, nch = fb.shape
+    offset = np.ascontiguousarray(offset, dtype=np.float32).reshape(ndm, nch)
+    scale = np.ascontiguousarray(scale, dtype=np.float32).reshape(ndm, nch)
+    codes = np.empty((ndm, nt, nch), np.uint8)
+    rc = lib().oracle_quantize(fb.ctypes.data, ndm, nt, nch, offset.ctypes.data, scale.ctypes.data, codes.ctypes.data)
+    if rc:
+        raise ValueError("oracle_quantize rc=%d" % rc)
+    return codes
