@@ -162,6 +162,34 @@ int cdmt_forward_spectrum(cdmt_plan *plan, const void *d_in, long long nsamp,
                           long long in_stride_pol, void *d_spec, void *d_workspace,
                           size_t workspace_bytes, void *cuda_stream);
 
+/*
+ * Redigitisation of one batch of filterbanks to 8 bit: Alg. 1 l.104-106 "compute block sums",
+ * "compute channel statistics", "redigitize".
+ *   d_fb          DEVICE float32, the output of cdmt_execute for `nblock` blocks: DM plane d at
+ *                 d * fb_stride_dm elements, [nblock*Vd][nsub*nchan] inside a plane.  Read only.
+ *   nblock        blocks in the batch (>= 1); statistics are taken per DM trial and per channel
+ *                 over the nblock*Vd samples of the batch
+ *   qmean, qstd   mean and standard deviation the codes of a channel shall have (qstd > 0).  The
+ *                 paper does not print its mapping; this library uses
+ *                     scale = std / qstd (1 if std == 0),  offset = mean - qmean * scale,
+ *                     code  = clip(rint((I - offset) / scale), 0, 255)
+ *                 with mean and population std from the per-block sums of I and I^2 (fp64), offset
+ *                 and scale rounded to float32, and the decision taken in float32 (IEEE subtract
+ *                 and divide, round half to even).
+ *   d_codes       DEVICE uint8, plane d at d * codes_stride_dm bytes, same [time][channel] order
+ *   d_offset, d_scale   DEVICE float32 [ndm][nsub*nchan] (dense), written
+ *   d_workspace   DEVICE scratch, 256-byte aligned, >= cdmt_redigitize_workspace_bytes():
+ *                 the block sums [ndm][nblock][nsub*nchan] x (sum I, sum I^2) in fp64
+ *   cuda_stream   cudaStream_t; three kernels are queued, nothing is synchronised
+ * Errors: CDMT_ERR_ARG (null / misaligned pointer, qstd <= 0), CDMT_ERR_SIZE (nblock < 1, stride
+ * shorter than a plane), CDMT_ERR_WORKSPACE, CDMT_ERR_CUDA.
+ */
+int cdmt_redigitize(cdmt_plan *plan, const float *d_fb, long long fb_stride_dm, long long nblock,
+                    double qmean, double qstd, unsigned char *d_codes, long long codes_stride_dm,
+                    float *d_offset, float *d_scale, void *d_workspace, size_t workspace_bytes,
+                    void *cuda_stream);
+int cdmt_redigitize_workspace_bytes(const cdmt_plan *plan, long long nblock, size_t *workspace_bytes);
+
 /* Eq. 2: dispersion sweep across [fcen - bw/2, fcen + bw/2] in seconds. */
 double cdmt_sweep_seconds(double fcen_mhz, double bw_mhz, double dm);
 /* smallest legal noverlap (input samples, rounded up to a multiple of 2 nchan)

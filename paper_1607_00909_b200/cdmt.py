@@ -26,7 +26,8 @@ OPT_FUSED_KERNEL = 4  # 0 auto, 1 general, 2 scalar fast, 3 packed half transfor
 EXPORTS = [
     "cdmt_plan_create", "cdmt_plan_destroy", "cdmt_plan_set_option", "cdmt_plan_query",
     "cdmt_execute", "cdmt_execute_host", "cdmt_host_scratch_bytes", "cdmt_host_traffic_bytes", "cdmt_unpack",
-    "cdmt_forward_spectrum", "cdmt_sweep_seconds", "cdmt_min_overlap",
+    "cdmt_forward_spectrum", "cdmt_redigitize", "cdmt_redigitize_workspace_bytes",
+    "cdmt_sweep_seconds", "cdmt_min_overlap",
     "cdmt_measure_fp32_peak", "cdmt_last_launch_count", "cdmt_profile_read", "cdmt_strerror",
     "cdmt_version",
 ]
@@ -51,6 +52,8 @@ _lib.cdmt_host_scratch_bytes.argtypes = [_vp, _ll, C.POINTER(_sz)]
 _lib.cdmt_host_traffic_bytes.argtypes = [_vp, _ll, C.POINTER(_sz), C.POINTER(_sz)]
 _lib.cdmt_unpack.argtypes = [_vp, _vp, _ll, _ll, _vp, _vp]
 _lib.cdmt_forward_spectrum.argtypes = [_vp, _vp, _ll, _ll, _vp, _vp, _sz, _vp]
+_lib.cdmt_redigitize.argtypes = [_vp, _vp, _ll, _ll, _d, _d, _vp, _ll, _vp, _vp, _vp, _sz, _vp]
+_lib.cdmt_redigitize_workspace_bytes.argtypes = [_vp, _ll, C.POINTER(_sz)]
 _lib.cdmt_sweep_seconds.argtypes = [_d, _d, _d]
 _lib.cdmt_sweep_seconds.restype = _d
 _lib.cdmt_min_overlap.argtypes = [_vp]
@@ -190,6 +193,21 @@ def cdmt_forward_spectrum(plan: Plan, d_in, nsamp: int, in_stride_pol: int, d_sp
     st = _lib.cdmt_forward_spectrum(plan.handle, _ptr(d_in), int(nsamp), int(in_stride_pol), _ptr(d_spec),
                                     _ptr(d_workspace), int(workspace_bytes), _stream(stream))
     _check(st, "cdmt_forward_spectrum")
+
+
+def cdmt_redigitize_workspace_bytes(plan: Plan, nblock: int) -> int:
+    n = _sz()
+    _check(_lib.cdmt_redigitize_workspace_bytes(plan.handle, int(nblock), C.byref(n)),
+           "cdmt_redigitize_workspace_bytes")
+    return n.value
+
+
+def cdmt_redigitize(plan: Plan, d_fb, fb_stride_dm: int, nblock: int, qmean: float, qstd: float, d_codes,
+                    codes_stride_dm: int, d_offset, d_scale, d_workspace, workspace_bytes: int, stream=None):
+    st = _lib.cdmt_redigitize(plan.handle, _ptr(d_fb), int(fb_stride_dm), int(nblock), float(qmean), float(qstd),
+                              _ptr(d_codes), int(codes_stride_dm), _ptr(d_offset), _ptr(d_scale),
+                              _ptr(d_workspace), int(workspace_bytes), _stream(stream))
+    _check(st, "cdmt_redigitize")
 
 
 def cdmt_min_overlap(plan: Plan) -> int:

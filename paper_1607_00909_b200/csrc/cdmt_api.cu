@@ -528,6 +528,37 @@ extern "C" int cdmt_execute_host(cdmt_plan *plan, const void *h_in, long long ns
     return r1 ? r1 : (r2 ? r2 : r3);
 }
 
+// ---- redigitisation (Alg. 1 l.104-106) ---------------------------------------------------
+extern "C" int cdmt_redigitize_workspace_bytes(const cdmt_plan *plan, long long nblock, size_t *workspace_bytes)
+{
+    if (!plan || !workspace_bytes) return CDMT_ERR_ARG;
+    if (nblock < 1 || nblock > 65535) return CDMT_ERR_SIZE;
+    *workspace_bytes = redigitize_workspace_bytes(plan->g, nblock);
+    return CDMT_OK;
+}
+
+extern "C" int cdmt_redigitize(cdmt_plan *plan, const float *d_fb, long long fb_stride_dm, long long nblock,
+                               double qmean, double qstd, unsigned char *d_codes, long long codes_stride_dm,
+                               float *d_offset, float *d_scale, void *d_workspace, size_t workspace_bytes,
+                               void *cuda_stream)
+{
+    if (!plan || !d_fb || !d_codes || !d_offset || !d_scale || !d_workspace) return CDMT_ERR_ARG;
+    if (!(qstd > 0.0) || !std::isfinite(qstd) || !std::isfinite(qmean)) return CDMT_ERR_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_fb) & 3) != 0 || (reinterpret_cast<uintptr_t>(d_offset) & 3) != 0 ||
+        (reinterpret_cast<uintptr_t>(d_scale) & 3) != 0 || (reinterpret_cast<uintptr_t>(d_workspace) & 255) != 0)
+        return CDMT_ERR_ARG;
+    const Geometry &g = plan->g;
+    if (nblock < 1 || nblock > 65535 || g.ndm > 65535) return CDMT_ERR_SIZE;
+    const long long plane = nblock * g.vdec * (long long)g.nsub * g.nchan;
+    if (fb_stride_dm < plane || codes_stride_dm < plane) return CDMT_ERR_SIZE;
+    if (nblock * g.vdec > 65535LL * 16) return CDMT_ERR_SIZE;
+    if (workspace_bytes < redigitize_workspace_bytes(g, nblock)) return CDMT_ERR_WORKSPACE;
+    plan->last_launches = 0;
+    return check_cuda(launch_redigitize(g, d_fb, fb_stride_dm, nblock, qmean, qstd, d_codes, codes_stride_dm, d_offset,
+                                        d_scale, d_workspace, static_cast<cudaStream_t>(cuda_stream),
+                                        &plan->last_launches));
+}
+
 // n_d n_c >= r t_d for the lowest-frequency channel (or subband) at the largest |DM|.
 extern "C" long long cdmt_min_overlap(const cdmt_plan *plan)
 {

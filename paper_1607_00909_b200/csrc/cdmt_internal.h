@@ -46,6 +46,13 @@ cudaError_t launch_unpack(const Geometry &g, const void *d_in, long long in_stri
                           int nblock, float2 *d_blocks, cudaStream_t st, long long *launches);
 cudaError_t launch_fp32_peak(float *d_scratch, int nblocks, int inner, cudaStream_t st);
 
+// cdmt_redigitize.cu: Alg. 1 l.104-106
+size_t redigitize_workspace_bytes(const Geometry &g, long long nblock);
+cudaError_t launch_redigitize(const Geometry &g, const float *d_fb, long long fb_stride_dm, long long nblock,
+                              double qmean, double qstd, unsigned char *d_codes, long long codes_stride_dm,
+                              float *d_offset, float *d_scale, void *d_workspace, cudaStream_t st,
+                              long long *launches);
+
 bool forward_len_supported(int L);
 bool fused_len_supported(int M);
 
