@@ -201,6 +201,7 @@ def main():
     ap.add_argument("--dm-tile", type=int, default=0)
     ap.add_argument("--fused-kernel", type=int, default=0, help="CDMT_OPT_FUSED_KERNEL (0 = library default)")
     ap.add_argument("--gen-threads", type=int, default=0)
+    ap.add_argument("--no-redigitize", action="store_true", help="skip the extra cdmt_redigitize timing (N1)")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -338,6 +339,42 @@ def main():
                 "share_of_step": prof["ms_fused"] / ms,
                 "forward_fft_ms_per_step": prof["ms_forward"] / args.steps}
 
+    # ---- extra (not part of `value`): 8-bit redigitisation of the filterbanks just computed
+    # (Alg. 1 l.104-106); HBM bound: 4 + 4 bytes read and 1 byte written per filterbank sample
+    redig = None
+    if not args.no_redigitize and groups == 1:
+        try:
+            nws = cdmt.cdmt_redigitize_workspace_bytes(plan, nb_total)
+            d_codes = torch.empty((cfg.ndm, nt, nch), dtype=torch.uint8, device=dev)
+            d_off = torch.empty((cfg.ndm, nch), dtype=torch.float32, device=dev)
+            d_sc = torch.empty((cfg.ndm, nch), dtype=torch.float32, device=dev)
+            d_rws = torch.empty(nws, dtype=torch.uint8, device=dev)
+            r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            reps = 3
+            for i in range(reps + 1):
+                if i == 1:
+                    r0.record(stream)
+                cdmt.cdmt_redigitize(plan, out, out[0].numel(), nb_total, 64.0, 16.0, d_codes, d_codes[0].numel(),
+                                     d_off, d_sc, d_rws, nws, stream)
+            r1.record(stream)
+            torch.cuda.synchronize()
+            rms = r0.elapsed_time(r1) / reps
+            rbytes = 9.0 * out.numel()
+            peaks = {}
+            try:
+                peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+            except Exception:
+                pass
+            hbm = float(peaks.get("hbm_gbs", 0)) or None
+            redig = {"ms_per_call": rms, "bytes": rbytes, "achieved_gbs": rbytes / rms / 1e6,
+                     "peak_gbs": hbm, "frac": (rbytes / rms / 1e6 / hbm) if hbm else None,
+                     "peak_source": "MEASURED_PEAKS.json hbm_gbs" if hbm else "unavailable",
+                     "launches": int(cdmt.cdmt_last_launch_count(plan)),
+                     "note": "cdmt_redigitize on the step's filterbanks; not included in value"}
+            del d_codes, d_rws
+        except Exception as e:   # never lose the headline line to the extra leg
+            redig = {"error": str(e)}
+
     # ---- end to end through the host-buffer entry point (pinned host memory, copies timed)
     e2e = None
     if want_e2e:
@@ -383,7 +420,7 @@ def main():
             "config": workload_config(cfg, args),
             "real_time_factor": cfg.nsamp * synth.TSAMP_S / sec_per_step,
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
-            "roofline": roofline, "cpu_baseline": cpu,
+            "roofline": roofline, "cpu_baseline": cpu, "redigitize": redig,
             "gen_seconds": t_gen, "out_groups": groups,
         }
         print(json.dumps(line), flush=True)
