@@ -422,10 +422,11 @@ cudaError_t launch_fused(const Geometry &g, const Workspace &ws, const float2 *s
     // 4 packed pols (pp), 5 packed pols, software-pipelined chirp (sp)
     const bool fast_ok = !accurate && M >= 512 && D <= 32 && (1 << logd) == D && (g.hdisc % D) == 0 &&
                          poly_phase_ok(g, h_dm, h_fcen);
-    const bool x2_ok = fast_ok && fused_x2_supported(M, D, g.hdisc);
+    // x2 and sp reduce the phase mod 1 with a 2^20 magic number: |phase| must stay below 2^19 cycles
+    const bool small_phase = phase_cycles_bound(g, h_dm, h_fcen) < 262144.0;
+    const bool x2_ok = fast_ok && small_phase && fused_x2_supported(M, D, g.hdisc);
     const bool pp_ok = fast_ok && fused_pp_supported(M, D, g.hdisc);
-    // sp reduces the phase mod 1 with a 2^20 magic number: |phase| must stay below 2^19 cycles
-    const bool sp_ok = fast_ok && fused_sp_supported(M, D, g.hdisc) && phase_cycles_bound(g, h_dm, h_fcen) < 262144.0;
+    const bool sp_ok = fast_ok && small_phase && fused_sp_supported(M, D, g.hdisc);
     if (force_generic == 5 && !sp_ok) return cudaErrorInvalidValue;
     if (sp_ok && (force_generic == 0 || force_generic == 5)) return launch_fused_sp(M, logd, fa, h_dm, nunits, st, launches);
     if (force_generic == 4 && !pp_ok) return cudaErrorInvalidValue;

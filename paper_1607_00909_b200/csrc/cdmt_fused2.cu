@@ -67,12 +67,35 @@ __device__ __forceinline__ float4 c2_to_f4(const C2 &v)
 }
 __device__ __forceinline__ C2 f4_to_c2(const float4 &q) { return C2{pk(q.x, q.y), pk(q.z, q.w)}; }
 
-// fractional part in [-0.5, 0.5] of a phase in cycles
-__device__ __forceinline__ float frac_of(double phi)
+// unit phasor of a phase in cycles (|phi| < 2^19, checked on the host): adding 1.5 * 2^20 leaves
+// round(phi * 2^32) mod 2^32 in the low mantissa word -- the fraction of a cycle as a signed
+// fixed-point number -- so one DADD reduces mod 1 and converts; I2FP, then MUFU sin/cos
+__device__ __forceinline__ float2 phasor_of(double phi)
 {
-    const double magic = 6755399441055744.0;  // 1.5 * 2^52
-    const double n = (phi + magic) - magic;
-    return (float)(phi - n);
+    const int frac32 = __double2loint(phi + 1572864.0);
+    const float x = __int2float_rn(frac32) * 1.4629180792671596e-9f;  // 2 pi / 2^32
+    return make_float2(__cosf(x), __sinf(x));
+}
+
+// Chirp of one DM trial on the thread's 16 x 2 bins (even bins in the low lane, odd in the high)
+template <int NT>
+__device__ __forceinline__ void x2_chirp(const double *coef, int tid, double dm, P2 (&Hr)[16], P2 (&Hi)[16])
+{
+    double pe[6], po[6];
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        pe[k] = dm * coef[(size_t)k * NT + tid];
+        po[k] = dm * coef[(size_t)(6 + k) * NT + tid];
+    }
+#pragma unroll
+    for (int r = 0; r < 16; ++r) {
+        const double rr = (double)r;
+        const double phe = fma(fma(fma(fma(fma(pe[5], rr, pe[4]), rr, pe[3]), rr, pe[2]), rr, pe[1]), rr, pe[0]);
+        const double pho = fma(fma(fma(fma(fma(po[5], rr, po[4]), rr, po[3]), rr, po[2]), rr, po[1]), rr, po[0]);
+        const float2 he = phasor_of(phe), ho = phasor_of(pho);
+        Hr[r] = pk(he.x, ho.x);
+        Hi[r] = pk(he.y, ho.y);
+    }
 }
 
 template <int M, int LOGD>
@@ -88,8 +111,9 @@ k_fused_x2(const FusedArgs a, const __grid_constant__ DmParams dmp)
     float4 *ex0 = smem4, *ex1 = smem4 + G::EX;
     float2 *integ = reinterpret_cast<float2 *>(smem4 + 2 * G::EX);
     double *coef = reinterpret_cast<double *>(integ + G::NWARP * G::INTEG);  // [2][6][NT]
-    uint64_t *bar = reinterpret_cast<uint64_t *>(coef + 12 * NT);
-    uint32_t *tslot = reinterpret_cast<uint32_t *>(bar + 1);
+    uint64_t *bar = reinterpret_cast<uint64_t *>(coef + 12 * NT);  // pass-2 loads done (buffers free)
+    uint64_t *barA = bar + 1;                                      // pass-1 stores done
+    uint32_t *tslot = reinterpret_cast<uint32_t *>(barA + 1);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int c = blockIdx.x % a.nchan;
@@ -97,7 +121,10 @@ k_fused_x2(const FusedArgs a, const __grid_constant__ DmParams dmp)
     const int unit = a.unit0 + ulocal, b = unit / a.nsub, s = unit % a.nsub;
 
     if (warp == 0) tmem_alloc<G::TCOLS>(tslot);
-    if (tid == 0) mbar_init(bar, NT);
+    if (tid == 0) {
+        mbar_init(bar, NT);
+        mbar_init(barA, NT);
+    }
     tmem_fence_before_sync();
     __syncthreads();
     tmem_fence_after_sync();
@@ -186,32 +213,17 @@ k_fused_x2(const FusedArgs a, const __grid_constant__ DmParams dmp)
     const int d_end = min(a.ndm, d_begin + a.dm_tile);
     float2 *ib = integ + warp * G::INTEG;
     __syncthreads();
+    // the chirp of trial d+1 is formed in the shadow of the block barrier of trial d and stays in
+    // registers (the data registers are dead there); the first one is formed here
+    P2 Hr[16], Hi[16];
+    if (d_begin < d_end) x2_chirp<NT>(coef, tid, dmp.dm[d_begin - a.dm_param0], Hr, Hi);
 
 #pragma unroll 1
     for (int d = d_begin; d < d_end; ++d) {
-        const double dm = dmp.dm[d - a.dm_param0];
-        // ---- chirp of this trial on the thread's 16 x 2 bins
-        P2 Hr[16], Hi[16];
-        {
-            double pe[6], po[6];
-#pragma unroll
-            for (int k = 0; k < 6; ++k) {
-                pe[k] = dm * coef[(size_t)k * NT + tid];
-                po[k] = dm * coef[(size_t)(6 + k) * NT + tid];
-            }
-#pragma unroll
-            for (int r = 0; r < 16; ++r) {
-                const double rr = (double)r;
-                const double phe = fma(fma(fma(fma(fma(pe[5], rr, pe[4]), rr, pe[3]), rr, pe[2]), rr, pe[1]), rr, pe[0]);
-                const double pho = fma(fma(fma(fma(fma(po[5], rr, po[4]), rr, po[3]), rr, po[2]), rr, po[1]), rr, po[0]);
-                const float2 he = unit_phasor<false>(frac_of(phe)), ho = unit_phasor<false>(frac_of(pho));
-                Hr[r] = pk(he.x, ho.x);
-                Hi[r] = pk(he.y, ho.y);
-            }
-        }
+        const unsigned par = (unsigned)(d - d_begin) & 1u;
         // ---- pass 0: both polarisations (the exchange buffers are free once every thread has
         //      finished the last pass of the previous trial)
-        if (d != d_begin) mbar_wait(bar, (unsigned)(d - d_begin - 1) & 1u);
+        if (d != d_begin) mbar_wait(bar, par ^ 1u);
 #pragma unroll
         for (int pol = 0; pol < 2; ++pol) {
             unsigned xr[64];
@@ -243,7 +255,9 @@ k_fused_x2(const FusedArgs a, const __grid_constant__ DmParams dmp)
                 for (int t1 = 0; t1 < 16; ++t1) p[t1 * G::PITCH] = c2_to_f4(v[t1]);
             }
         }
-        __syncthreads();
+        mbar_arrive(barA);
+        if (d + 1 < d_end) x2_chirp<NT>(coef, tid, dmp.dm[d + 1 - a.dm_param0], Hr, Hi);
+        mbar_wait(barA, par);
         // ---- pass 2 along j2, radix-2 combine, detection, polarisation sum
         P2 pw[16];  // (|y[t']|^2, |y[t' + L]|^2) summed over polarisations, order k = u R2 + t2
         {
