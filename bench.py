@@ -35,8 +35,8 @@ UNIT = "samples*DM/s"
 # (unit counts and clocks: /opt/skills/guides/B200_PROFILING.md, MEASURED_PEAKS.json sm_max_mhz)
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 # DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per fused-kernel launch from the committed
-# `ncu --set full` capture (profiles/r1_sp_c3.md: 1.084882 + 1.168516 GB; c3, default chunking)
-FUSED_TRAFFIC_BYTES_PER_LAUNCH = {"c3": 2253398000}
+# `ncu --set full` capture (profiles/r1_x2_c3.md: 1.085494 + 1.168215 GB; c3, default chunking)
+FUSED_TRAFFIC_BYTES_PER_LAUNCH = {"c3": 2253709000}
 
 
 def algorithmic_flops_per_unit_dm(cfg: synth.Config) -> float:
@@ -331,7 +331,7 @@ def main():
     roofline = {"bound": "alu", "kernel": "k_fused", "achieved": achieved, "peak": FP32_PEAK_TFLOPS,
                 "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
                 "traffic": FUSED_TRAFFIC_BYTES_PER_LAUNCH.get(cfg.name) if not (args.chunk_units or args.dm_tile) else None,
-                "traffic_source": "profiles/r1_sp_c3.md (ncu --set full, one launch)",
+                "traffic_source": "profiles/r1_x2_c3.md (ncu --set full, one launch)",
                 "peak_source": "derived: 148 SM x 128 lanes x 2 x 1.965 GHz",
                 "fma_peak_measured_tflops": fma_peak,
                 "ms_per_launch": ms_per_launch, "launches_timed": prof["n_fused"],

@@ -428,12 +428,14 @@ cudaError_t launch_fused(const Geometry &g, const Workspace &ws, const float2 *s
     const bool pp_ok = fast_ok && fused_pp_supported(M, D, g.hdisc);
     const bool sp_ok = fast_ok && small_phase && fused_sp_supported(M, D, g.hdisc);
     if (force_generic == 5 && !sp_ok) return cudaErrorInvalidValue;
-    if (sp_ok && (force_generic == 0 || force_generic == 5)) return launch_fused_sp(M, logd, fa, h_dm, nunits, st, launches);
     if (force_generic == 4 && !pp_ok) return cudaErrorInvalidValue;
     if (force_generic == 3 && !x2_ok) return cudaErrorInvalidValue;
     if (force_generic == 2 && !fast_ok) return cudaErrorInvalidValue;
-    if (pp_ok && (force_generic == 0 || force_generic == 4)) return launch_fused_pp(M, logd, fa, h_dm, nunits, st, launches);
+    // automatic choice: x2 (measured fastest on all five configs: c3 21.8 ms per launch against 22.2 for sp),
+    // then sp (covers ndec < 8), then pp
     if (x2_ok && (force_generic == 0 || force_generic == 3)) return launch_fused_x2(M, logd, fa, h_dm, nunits, st, launches);
+    if (sp_ok && (force_generic == 0 || force_generic == 5)) return launch_fused_sp(M, logd, fa, h_dm, nunits, st, launches);
+    if (pp_ok && (force_generic == 0 || force_generic == 4)) return launch_fused_pp(M, logd, fa, h_dm, nunits, st, launches);
     const bool fast = fast_ok && force_generic != 1;
     cudaError_t e = cudaErrorInvalidValue;
     if (fast) {
