@@ -408,3 +408,60 @@ int oracle_quantize(const float *fb, long ndm, long nt, long nch, const float *o
             }
     return 0;
 }
+
+/* ------------------------------------------------------------------------------------------
+ * Incoherent dedispersion of ONE coherently dedispersed filterbank over a grid of fine DM
+ * offsets: the second stage of the semi-coherent search of PAPER.md:35 and PAPER.md:141
+ * ("each of the coherently dedispersed filterbanks was then incoherently dedispersed at steps
+ * of 0.002 pc cm^-3 ranging from -0.5 to 0.5 pc cm^-3 around the coherently dedispersed DM ...
+ * brute force dedispersion algorithm").  The paper uses a third-party library and prints no
+ * formula beyond Eq. 2; the brute-force definition is written out here (readings Q23-Q26):
+ *
+ *   channel j of the filterbank (DESCENDING frequency) has centre frequency f_j;
+ *   the residual delay of channel j at DM offset ddm relative to the highest channel f_0 is
+ *       tau_j = ddm (f_j^-2 - f_0^-2) / 2.41e-4   seconds   (Eq. 2 between two frequencies, MHz)
+ *   shift[k][j] = rint(tau_j(ddm_k) / tsamp)       samples (round half to even, fp64)
+ *   smin, smax  = extremes of shift over all k, j (smin <= 0 <= smax: shift[k][0] = 0)
+ *   ts[k][t]    = sum_j fb[t + shift[k][j] - smin][j],   t < nt - (smax - smin)
+ *
+ * so output sample t is time t - smin of the highest channel, and only samples for which
+ * every channel is inside the filterbank are produced (valid-only, as reading Q8).
+ * The sum over channels is taken in double, in channel order, and rounded to float32 last.
+ *
+ *   fb      [nt][nch] float32       fch [nch] channel centre frequencies, MHz
+ *   ddm     [nfine]                 tsamp: filterbank sample time, seconds
+ *   shifts  [nfine][nch] int32 (may be NULL), ts [nfine][nt - (smax-smin)] float32 (may be NULL)
+ * Returns smax - smin in *range and smin in *smin_out (either may be NULL); nonzero on error.
+ */
+int oracle_incoherent(const float *fb, long nt, long nch, const double *fch, double tsamp, long nfine,
+                      const double *ddm, int *shifts, float *ts, long *range, long *smin_out)
+{
+    if (nt < 1 || nch < 1 || nfine < 1 || !fch || !ddm || !(tsamp > 0.0)) return 1;
+    int *sh = shifts ? shifts : (int *)malloc(sizeof(int) * (size_t)nfine * nch);
+    if (!sh) return 2;
+    long smin = 0, smax = 0;
+    for (long k = 0; k < nfine; k++)
+        for (long j = 0; j < nch; j++) {
+            const double tau = ddm[k] * (1.0 / (fch[j] * fch[j]) - 1.0 / (fch[0] * fch[0])) / KDM_INV_S_MHZ2;
+            const long s = (long)nearbyint(tau / tsamp);
+            sh[k * nch + j] = (int)s;
+            if (s < smin) smin = s;
+            if (s > smax) smax = s;
+        }
+    if (range) *range = smax - smin;
+    if (smin_out) *smin_out = smin;
+    int rc = 0;
+    const long nout = nt - (smax - smin);
+    if (ts) {
+        if (!fb || nout < 1) rc = 3;
+        else
+            for (long k = 0; k < nfine; k++)
+                for (long t = 0; t < nout; t++) {
+                    double acc = 0.0;
+                    for (long j = 0; j < nch; j++) acc += (double)fb[(size_t)(t + sh[k * nch + j] - smin) * nch + j];
+                    ts[(size_t)k * nout + t] = (float)acc;
+                }
+    }
+    if (!shifts) free(sh);
+    return rc;
+}

@@ -64,6 +64,8 @@ def lib():
         L.oracle_channel_timeseries.argtypes = [C.POINTER(_Params), C.c_int, C.c_int, C.c_double,
                                                 C.c_void_p, C.c_void_p]
         L.oracle_redigitize.argtypes = [C.c_void_p] + [C.c_long] * 4 + [C.c_double] * 2 + [C.c_void_p] * 6
+        L.oracle_incoherent.argtypes = [C.c_void_p, C.c_long, C.c_long, C.c_void_p, C.c_double, C.c_long,
+                                        C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_long), C.POINTER(C.c_long)]
         L.oracle_quantize.argtypes = [C.c_void_p] + [C.c_long] * 3 + [C.c_void_p] * 3
         _lib = L
     return _lib
@@ -213,3 +215,35 @@ def quantize(fb: np.ndarray, offset: np.ndarray, scale: np.ndarray) -> np.ndarra
     if rc:
         raise ValueError("oracle_quantize rc=%d" % rc)
     return codes
+
+
+def channel_frequencies(p: Params) -> np.ndarray:
+    """Centre frequencies (MHz) of the filterbank channels in OUTPUT order (descending)."""
+    c = np.arange(p.nchan)
+    f = (p.fcen[:, None] + (c[None, :] + 0.5 - p.nchan / 2) * p.bw_mhz / p.nchan).reshape(-1)
+    return np.ascontiguousarray(f[::-1])
+
+
+def incoherent(fb: np.ndarray, fch: np.ndarray, tsamp: float, ddm, want_ts: bool = True) -> dict:
+    """Brute-force incoherent dedispersion of one filterbank fb [nt][nch] over fine DM offsets ddm
+    (PAPER.md:141).  Returns dict(shifts [nfine][nch] int32, smin, range, ts [nfine][nt-range] float32)."""
+    fb = np.ascontiguousarray(fb, dtype=np.float32)
+    nt, nch = fb.shape
+    fch = np.ascontiguousarray(fch, dtype=np.float64)
+    ddm = np.ascontiguousarray(ddm, dtype=np.float64).reshape(-1)
+    assert fch.size == nch
+    shifts = np.empty((ddm.size, nch), np.int32)
+    rng, smin = C.c_long(), C.c_long()
+    rc = lib().oracle_incoherent(fb.ctypes.data, nt, nch, fch.ctypes.data, float(tsamp), ddm.size, ddm.ctypes.data,
+                                 shifts.ctypes.data, None, C.byref(rng), C.byref(smin))
+    if rc:
+        raise ValueError("oracle_incoherent rc=%d" % rc)
+    out = dict(shifts=shifts, smin=smin.value, range=rng.value, ts=None)
+    if want_ts:
+        ts = np.empty((ddm.size, nt - rng.value), np.float32)
+        rc = lib().oracle_incoherent(fb.ctypes.data, nt, nch, fch.ctypes.data, float(tsamp), ddm.size, ddm.ctypes.data,
+                                     shifts.ctypes.data, ts.ctypes.data, None, None)
+        if rc:
+            raise ValueError("oracle_incoherent rc=%d" % rc)
+        out["ts"] = ts
+    return out
