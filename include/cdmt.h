@@ -190,6 +190,39 @@ int cdmt_redigitize(cdmt_plan *plan, const float *d_fb, long long fb_stride_dm, 
                     void *cuda_stream);
 int cdmt_redigitize_workspace_bytes(const cdmt_plan *plan, long long nblock, size_t *workspace_bytes);
 
+/*
+ * Incoherent dedispersion of the coherently dedispersed filterbanks over a grid of fine DM offsets:
+ * the second stage of the semi-coherent search ("each of the coherently
+ * dedispersed filterbanks was then incoherently dedispersed at steps of 0.002 pc cm^-3 ranging
+ * from -0.5 to 0.5 pc cm^-3 around the coherently dedispersed DM ... brute force dedispersion").
+ * With f_j the centre of filterbank channel j (descending order, f_0 the highest) and tsamp =
+ * nchan * ndec / bw the filterbank sample time,
+ *     shift[k][j] = rint(ddm[k] * (f_j^-2 - f_0^-2) / 2.41e-4 / tsamp)          (Eq. 2; fp64, half to even)
+ *     ts[d][k][t] = sum_j fb[d][t + shift[k][j] - shift_min][j],  t < nt_out = nt_in - shift_range
+ * (valid-only: output sample t is time t - shift_min of the highest channel).  The same offsets are
+ * applied to every coherent DM plane d.
+ *   nfine, ddm     HOST [nfine] DM offsets in pc cm^-3, strictly ascending; copied
+ *   d_fb           DEVICE float32, plane d at d * fb_stride_dm elements, [nt_in][nsub*nchan] inside
+ *   d_ts           DEVICE float32, plane d at d * ts_stride_dm elements, row k at k * ts_pitch,
+ *                  nt_out samples per row (ts_pitch >= nt_out, ts_stride_dm >= nfine * ts_pitch)
+ *   d_workspace    DEVICE scratch, 256-byte aligned, >= workspace_bytes from cdmt_incoherent_query
+ * cdmt_incoherent_query: host arithmetic only; any output pointer may be NULL.  ngroups = number
+ * of trial groups the kernel works in (<= 16 trials each; fewer where the shifts of consecutive
+ * trials differ by more than the kernel's register window allows).
+ * cdmt_incoherent_shifts: copies the shift table [nfine][nsub*nchan] to HOST memory.
+ * Sums are accumulated in float32 in channel order.
+ * Errors: CDMT_ERR_ARG (null / misaligned pointer, non-finite or non-ascending ddm), CDMT_ERR_SIZE
+ * (nt_in <= shift_range, short strides), CDMT_ERR_WORKSPACE, CDMT_ERR_ALLOC, CDMT_ERR_CUDA.
+ */
+int cdmt_incoherent_query(cdmt_plan *plan, int nfine, const double *ddm, long long nt_in,
+                          int *shift_min, int *shift_range, long long *nt_out, int *ngroups,
+                          size_t *workspace_bytes);
+int cdmt_incoherent_shifts(cdmt_plan *plan, int nfine, const double *ddm, int *h_shifts);
+int cdmt_incoherent_dedisperse(cdmt_plan *plan, const float *d_fb, long long fb_stride_dm,
+                               long long nt_in, int nfine, const double *ddm, float *d_ts,
+                               long long ts_stride_dm, long long ts_pitch, void *d_workspace,
+                               size_t workspace_bytes, void *cuda_stream);
+
 /* Eq. 2: dispersion sweep across [fcen - bw/2, fcen + bw/2] in seconds. */
 double cdmt_sweep_seconds(double fcen_mhz, double bw_mhz, double dm);
 /* smallest legal noverlap (input samples, rounded up to a multiple of 2 nchan)

@@ -27,6 +27,7 @@ EXPORTS = [
     "cdmt_plan_create", "cdmt_plan_destroy", "cdmt_plan_set_option", "cdmt_plan_query",
     "cdmt_execute", "cdmt_execute_host", "cdmt_host_scratch_bytes", "cdmt_host_traffic_bytes", "cdmt_unpack",
     "cdmt_forward_spectrum", "cdmt_redigitize", "cdmt_redigitize_workspace_bytes",
+    "cdmt_incoherent_query", "cdmt_incoherent_shifts", "cdmt_incoherent_dedisperse",
     "cdmt_sweep_seconds", "cdmt_min_overlap",
     "cdmt_measure_fp32_peak", "cdmt_last_launch_count", "cdmt_profile_read", "cdmt_strerror",
     "cdmt_version",
@@ -54,6 +55,10 @@ _lib.cdmt_unpack.argtypes = [_vp, _vp, _ll, _ll, _vp, _vp]
 _lib.cdmt_forward_spectrum.argtypes = [_vp, _vp, _ll, _ll, _vp, _vp, _sz, _vp]
 _lib.cdmt_redigitize.argtypes = [_vp, _vp, _ll, _ll, _d, _d, _vp, _ll, _vp, _vp, _vp, _sz, _vp]
 _lib.cdmt_redigitize_workspace_bytes.argtypes = [_vp, _ll, C.POINTER(_sz)]
+_lib.cdmt_incoherent_query.argtypes = [_vp, _i, C.POINTER(_d), _ll, C.POINTER(_i), C.POINTER(_i), C.POINTER(_ll),
+                                       C.POINTER(_i), C.POINTER(_sz)]
+_lib.cdmt_incoherent_shifts.argtypes = [_vp, _i, C.POINTER(_d), _vp]
+_lib.cdmt_incoherent_dedisperse.argtypes = [_vp, _vp, _ll, _ll, _i, C.POINTER(_d), _vp, _ll, _ll, _vp, _sz, _vp]
 _lib.cdmt_sweep_seconds.argtypes = [_d, _d, _d]
 _lib.cdmt_sweep_seconds.restype = _d
 _lib.cdmt_min_overlap.argtypes = [_vp]
@@ -208,6 +213,36 @@ def cdmt_redigitize(plan: Plan, d_fb, fb_stride_dm: int, nblock: int, qmean: flo
                               _ptr(d_codes), int(codes_stride_dm), _ptr(d_offset), _ptr(d_scale),
                               _ptr(d_workspace), int(workspace_bytes), _stream(stream))
     _check(st, "cdmt_redigitize")
+
+
+def _ddm(ddm):
+    a = np.ascontiguousarray(ddm, dtype=np.float64).reshape(-1)
+    return a, a.ctypes.data_as(C.POINTER(_d))
+
+
+def cdmt_incoherent_query(plan: Plan, ddm, nt_in: int) -> dict:
+    a, pa = _ddm(ddm)
+    smin, rng, ng, nout, nws = _i(), _i(), _i(), _ll(), _sz()
+    _check(_lib.cdmt_incoherent_query(plan.handle, a.size, pa, int(nt_in), C.byref(smin), C.byref(rng),
+                                      C.byref(nout), C.byref(ng), C.byref(nws)), "cdmt_incoherent_query")
+    return dict(shift_min=smin.value, shift_range=rng.value, nt_out=nout.value, ngroups=ng.value,
+                workspace_bytes=nws.value)
+
+
+def cdmt_incoherent_shifts(plan: Plan, ddm) -> np.ndarray:
+    a, pa = _ddm(ddm)
+    out = np.empty((a.size, plan.nsub * plan.nchan), dtype=np.int32)
+    _check(_lib.cdmt_incoherent_shifts(plan.handle, a.size, pa, out.ctypes.data), "cdmt_incoherent_shifts")
+    return out
+
+
+def cdmt_incoherent_dedisperse(plan: Plan, d_fb, fb_stride_dm: int, nt_in: int, ddm, d_ts, ts_stride_dm: int,
+                               ts_pitch: int, d_workspace, workspace_bytes: int, stream=None):
+    a, pa = _ddm(ddm)
+    st = _lib.cdmt_incoherent_dedisperse(plan.handle, _ptr(d_fb), int(fb_stride_dm), int(nt_in), a.size, pa,
+                                         _ptr(d_ts), int(ts_stride_dm), int(ts_pitch), _ptr(d_workspace),
+                                         int(workspace_bytes), _stream(stream))
+    _check(st, "cdmt_incoherent_dedisperse")
 
 
 def cdmt_min_overlap(plan: Plan) -> int:

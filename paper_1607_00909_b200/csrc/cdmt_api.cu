@@ -26,6 +26,8 @@ struct cdmt_plan {
     struct Span { size_t e0, e1; int kind; };   // kind 0: forward FFT passes, 1: fused per-DM kernel
     std::vector<Span> spans;
     // host-buffer path (cdmt_execute_host): copy streams and the events that order the double buffers
+    IncoherentTables ic;     // incoherent-dedispersion tables of the last fine-DM list used
+    std::vector<double> ic_ddm;
     cudaStream_t s_in, s_out;
     cudaEvent_t ev_start, ev_h2d[2], ev_comp[2], ev_d2h[2];
     bool host_ready;
@@ -557,6 +559,71 @@ extern "C" int cdmt_redigitize(cdmt_plan *plan, const float *d_fb, long long fb_
     return check_cuda(launch_redigitize(g, d_fb, fb_stride_dm, nblock, qmean, qstd, d_codes, codes_stride_dm, d_offset,
                                         d_scale, d_workspace, static_cast<cudaStream_t>(cuda_stream),
                                         &plan->last_launches));
+}
+
+// ---- incoherent dedispersion over fine DM offsets ----------------------------
+static int plan_incoherent(cdmt_plan *plan, int nfine, const double *ddm)
+{
+    if (!plan || !ddm) return CDMT_ERR_ARG;
+    if (nfine < 1 || nfine > (1 << 20)) return CDMT_ERR_SIZE;
+    for (int k = 0; k < nfine; ++k)
+        if (!std::isfinite(ddm[k])) return CDMT_ERR_ARG;
+    if ((int)plan->ic_ddm.size() == nfine && std::memcmp(plan->ic_ddm.data(), ddm, sizeof(double) * nfine) == 0)
+        return CDMT_OK;
+    try {
+        plan->ic_ddm.clear();
+        if (!incoherent_plan(plan->g, plan->fcen.data(), nfine, ddm, &plan->ic)) return CDMT_ERR_ARG;
+        plan->ic_ddm.assign(ddm, ddm + nfine);
+    } catch (...) {
+        plan->ic_ddm.clear();
+        return CDMT_ERR_ALLOC;
+    }
+    return CDMT_OK;
+}
+
+extern "C" int cdmt_incoherent_query(cdmt_plan *plan, int nfine, const double *ddm, long long nt_in, int *shift_min,
+                                     int *shift_range, long long *nt_out, int *ngroups, size_t *workspace_bytes)
+{
+    int rc = plan_incoherent(plan, nfine, ddm);
+    if (rc) return rc;
+    if (shift_min) *shift_min = plan->ic.smin;
+    if (shift_range) *shift_range = plan->ic.range;
+    if (nt_out) *nt_out = nt_in - plan->ic.range;
+    if (ngroups) *ngroups = (int)plan->ic.groups.size();
+    if (workspace_bytes) *workspace_bytes = incoherent_workspace_bytes(plan->ic);
+    return CDMT_OK;
+}
+
+extern "C" int cdmt_incoherent_shifts(cdmt_plan *plan, int nfine, const double *ddm, int *h_shifts)
+{
+    if (!h_shifts) return CDMT_ERR_ARG;
+    int rc = plan_incoherent(plan, nfine, ddm);
+    if (rc) return rc;
+    std::memcpy(h_shifts, plan->ic.shifts.data(), sizeof(int) * plan->ic.shifts.size());
+    return CDMT_OK;
+}
+
+extern "C" int cdmt_incoherent_dedisperse(cdmt_plan *plan, const float *d_fb, long long fb_stride_dm, long long nt_in,
+                                          int nfine, const double *ddm, float *d_ts, long long ts_stride_dm,
+                                          long long ts_pitch, void *d_workspace, size_t workspace_bytes,
+                                          void *cuda_stream)
+{
+    if (!plan || !d_fb || !d_ts || !d_workspace) return CDMT_ERR_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_fb) & 3) != 0 || (reinterpret_cast<uintptr_t>(d_ts) & 3) != 0 ||
+        (reinterpret_cast<uintptr_t>(d_workspace) & 255) != 0)
+        return CDMT_ERR_ARG;
+    int rc = plan_incoherent(plan, nfine, ddm);
+    if (rc) return rc;
+    const Geometry &g = plan->g;
+    const long long nch = (long long)g.nsub * g.nchan;
+    const long long nt_out = nt_in - plan->ic.range;
+    if (nt_in < 1 || nt_in > (1LL << 30) || nt_out < 1) return CDMT_ERR_SIZE;
+    if (fb_stride_dm < nt_in * nch || ts_pitch < nt_out || ts_stride_dm < (long long)nfine * ts_pitch) return CDMT_ERR_SIZE;
+    if (g.ndm > 65535 || (plan->ic.groups.size() + 3) / 4 > 65535) return CDMT_ERR_SIZE;
+    if (workspace_bytes < incoherent_workspace_bytes(plan->ic)) return CDMT_ERR_WORKSPACE;
+    plan->last_launches = 0;
+    return check_cuda(launch_incoherent(g, plan->ic, d_fb, fb_stride_dm, nt_in, d_ts, ts_stride_dm, ts_pitch,
+                                        d_workspace, static_cast<cudaStream_t>(cuda_stream), &plan->last_launches));
 }
 
 // n_d n_c >= r t_d for the lowest-frequency channel (or subband) at the largest |DM|.

@@ -4,6 +4,8 @@
 #include <stddef.h>
 #include <stdint.h>
 
+#include <vector>
+
 namespace cdmt {
 
 struct Geometry {
@@ -52,6 +54,21 @@ cudaError_t launch_redigitize(const Geometry &g, const float *d_fb, long long fb
                               double qmean, double qstd, unsigned char *d_codes, long long codes_stride_dm,
                               float *d_offset, float *d_scale, void *d_workspace, cudaStream_t st,
                               long long *launches);
+
+// cdmt_incoherent.cu: incoherent dedispersion of the filterbanks over fine DM offsets
+struct IncoherentTables {            // host side, owned by the plan (must outlive the async upload)
+    int nfine = 0, nch = 0;
+    int smin = 0, range = 0;         // extremes of the shift table: range = smax - smin
+    std::vector<int> shifts;         // [nfine][nch] samples, channel order of the filterbank (descending)
+    std::vector<uint2> entries;      // [ngroups][nch]: x = first trial's shift - smin, y = 2-bit increments
+    std::vector<int2> groups;        // [ngroups]: (first trial, number of trials <= 16)
+};
+// Fills the tables; returns false if ddm is not ascending.
+bool incoherent_plan(const Geometry &g, const double *h_fcen, int nfine, const double *ddm, IncoherentTables *T);
+size_t incoherent_workspace_bytes(const IncoherentTables &T);
+cudaError_t launch_incoherent(const Geometry &g, const IncoherentTables &T, const float *d_fb, long long fb_stride_dm,
+                              long long nt_in, float *d_ts, long long ts_stride_dm, long long ts_pitch,
+                              void *d_workspace, cudaStream_t st, long long *launches);
 
 bool forward_len_supported(int L);
 bool fused_len_supported(int M);
