@@ -202,6 +202,8 @@ def main():
     ap.add_argument("--fused-kernel", type=int, default=0, help="CDMT_OPT_FUSED_KERNEL (0 = library default)")
     ap.add_argument("--gen-threads", type=int, default=0)
     ap.add_argument("--no-redigitize", action="store_true", help="skip the extra cdmt_redigitize timing (N1)")
+    ap.add_argument("--no-incoherent", action="store_true", help="skip the extra cdmt_incoherent_dedisperse timing (N2)")
+    ap.add_argument("--fine-step", type=float, default=0.002, help="fine DM step of the incoherent leg (PAPER.md:141)")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -375,6 +377,41 @@ def main():
         except Exception as e:   # never lose the headline line to the extra leg
             redig = {"error": str(e)}
 
+    # ---- extra (not part of `value`): incoherent dedispersion of every coherent filterbank over fine DM
+    # offsets spanning the coherent DM step at PAPER.md:141's 0.002 pc/cm3 (semi-coherent search);
+    # FP32-add bound: one add per (coherent DM, fine trial, channel, output sample)
+    incoh = None
+    if not args.no_incoherent and groups == 1:
+        try:
+            dm_step = float(cfg.dm[1] - cfg.dm[0]) if cfg.ndm > 1 else 1.0
+            nhalf = int(round(0.5 * dm_step / args.fine_step))
+            ddm = np.round(np.arange(-nhalf, nhalf + 1) * args.fine_step, 9)
+            qi = cdmt.cdmt_incoherent_query(plan, ddm, nt)
+            d_ts = torch.empty((cfg.ndm, len(ddm), qi["nt_out"]), dtype=torch.float32, device=dev)
+            d_iws = torch.empty(max(256, qi["workspace_bytes"]), dtype=torch.uint8, device=dev)
+            i0, i1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            reps = 2
+            for i in range(reps + 1):
+                if i == 1:
+                    i0.record(stream)
+                cdmt.cdmt_incoherent_dedisperse(plan, out, out[0].numel(), nt, ddm, d_ts, d_ts[0].numel(),
+                                                qi["nt_out"], d_iws, d_iws.numel(), stream)
+            i1.record(stream)
+            torch.cuda.synchronize()
+            ims = i0.elapsed_time(i1) / reps
+            adds = float(cfg.ndm) * len(ddm) * nch * qi["nt_out"]
+            peak_add = 148 * 128 * 1.965e9 / 1e12
+            incoh = {"ms_per_call": ims, "fine_trials": len(ddm), "fine_step": args.fine_step,
+                     "trial_groups": qi["ngroups"], "shift_range": qi["shift_range"], "adds": adds,
+                     "achieved_tadd_s": adds / ims / 1e9, "peak_tadd_s": peak_add,
+                     "frac": adds / ims / 1e9 / peak_add, "bound": "alu",
+                     "peak_source": "derived: 148 SM x 128 FP32 lanes x 1.965 GHz (one FADD per lane and clock)",
+                     "out_bytes": int(d_ts.numel() * 4),
+                     "note": "cdmt_incoherent_dedisperse on the step's filterbanks; not included in value"}
+            del d_ts, d_iws
+        except Exception as e:
+            incoh = {"error": str(e)}
+
     # ---- end to end through the host-buffer entry point (pinned host memory, copies timed)
     e2e = None
     if want_e2e:
@@ -420,7 +457,7 @@ def main():
             "config": workload_config(cfg, args),
             "real_time_factor": cfg.nsamp * synth.TSAMP_S / sec_per_step,
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
-            "roofline": roofline, "cpu_baseline": cpu, "redigitize": redig,
+            "roofline": roofline, "cpu_baseline": cpu, "redigitize": redig, "incoherent": incoh,
             "gen_seconds": t_gen, "out_groups": groups,
         }
         print(json.dumps(line), flush=True)

@@ -8,15 +8,14 @@
 //
 // The filterbank is time-major, channel-fastest; dedispersion wants runs along time.
 // A CTA (4 warps) owns 256 output samples of 64 trials: it walks the channels in chunks of CC,
-// transposing each chunk's tile [CC][256 + range + ...] into shared memory (coalesced loads along
-// channels), and every warp adds the chunk into the 16 trials x 8 samples it keeps in registers.
-// Per channel a thread loads two 8-sample windows (4 x LDS.128) that serve all 16 trials of its
-// group: the host orders the trials by DM offset and cuts groups so that, inside a group, the shift
-// of any channel grows by at most 4 samples, so the window only ever slides forward by register
-// moves (2-bit increments per trial from a table).  Four copies of the tile, displaced by 0..3
-// samples, make every window start 16-byte aligned.  128 FADD per 16 floats read from shared memory:
-// the kernel is bound by the FP32 pipe, not by shared-memory bandwidth (4 adds per float would be
-// the break-even).
+// transposing each chunk's tile [CC][256 + range] into shared memory (coalesced loads along
+// channels), and every warp adds the chunk into the 16 trials x 8 samples (t = lane + 32 i) it
+// keeps in registers.  The host orders the trials by DM offset and cuts them into groups of 16, so
+// inside a group the shift of a channel only grows, and by little: per channel a thread reads its 8
+// samples at the first trial's shift (conflict-free LDS.32) and re-reads them only where a trial's
+// shift differs from the previous one (2-bit increments per trial from a table).  128 FADD per 8-24
+// floats read from shared memory: the kernel is bound by the FP32 pipe (4 adds per float read would
+// be the break-even with shared-memory bandwidth).
 #include <algorithm>
 #include <cmath>
 #include <cstdint>
@@ -28,7 +27,7 @@ namespace cdmt {
 constexpr int IC_TILE = 256;     // output samples per CTA
 constexpr int IC_GROUP = 16;     // trials per warp
 constexpr int IC_WARPS = 4;      // warps (trial groups) per CTA
-constexpr int IC_MAXSPREAD = 4;  // growth of a channel's shift inside a group the 8-sample window allows
+constexpr int IC_MAXSTEP = 3;    // largest growth of a channel's shift from one trial to the next (2-bit table field)
 
 // ------------------------------------------------------------------------------------------ host
 bool incoherent_plan(const Geometry &g, const double *h_fcen, int nfine, const double *ddm, IncoherentTables *T)
@@ -57,7 +56,7 @@ bool incoherent_plan(const Geometry &g, const double *h_fcen, int nfine, const d
         }
     T->smin = smin;
     T->range = smax - smin;
-    // groups of up to 16 consecutive trials whose shifts stay inside the sliding window
+    // groups of up to 16 consecutive trials whose shifts grow by at most 3 samples per trial
     T->groups.clear();
     T->entries.clear();
     int k0 = 0;
@@ -66,9 +65,8 @@ bool incoherent_plan(const Geometry &g, const double *h_fcen, int nfine, const d
         while (n < IC_GROUP && k0 + n < nfine) {
             bool ok = true;
             const int *a = &T->shifts[(size_t)(k0 + n) * nch], *p = &T->shifts[(size_t)(k0 + n - 1) * nch];
-            const int *b = &T->shifts[(size_t)k0 * nch];
             for (int j = 0; j < nch && ok; ++j)
-                ok = a[j] >= p[j] && a[j] - p[j] <= 3 && a[j] - b[j] <= IC_MAXSPREAD;
+                ok = a[j] >= p[j] && a[j] - p[j] <= IC_MAXSTEP;
             if (!ok) break;
             ++n;
         }
@@ -103,33 +101,34 @@ struct IcArgs {
     long long ts_stride_dm, ts_pitch;
     const uint2 *entries;   // [ngroups][nch]
     const int2 *groups;     // [ngroups]
-    int nt_in, nt_out, nch, ngroups, cc, tw, vec_in, vec_out;
+    int nt_in, nt_out, nch, ngroups, cc, tw, vec_in;
 };
 
-__device__ __forceinline__ void ic_slide(float (&v)[8])
+// this lane's 8 samples t = lane + 32 i of one channel at the current shift
+__device__ __forceinline__ void ic_window(float (&v)[8], const float *p)
 {
 #pragma unroll
-    for (int i = 0; i < 7; ++i) v[i] = v[i + 1];
+    for (int i = 0; i < 8; ++i) v[i] = p[32 * i];
 }
 
 // grid (ceil(nt_out / 256), ceil(ngroups / 4), ndm), 128 threads; dynamic shared memory:
-// float tile[cc][4 copies][tw] (+ skew) and uint2 tab[4][cc]
-__global__ void __launch_bounds__(32 * IC_WARPS, 2) k_incoherent(const IcArgs a)
+// float tile[cc][tw] and uint2 tab[4][cc]
+__global__ void __launch_bounds__(32 * IC_WARPS, 3) k_incoherent(const IcArgs a)
 {
     extern __shared__ float4 ic_smem4[];
     float *tile = reinterpret_cast<float *>(ic_smem4);
     const int cc = a.cc, tw = a.tw, quads = cc >> 2;
-    uint2 *tab = reinterpret_cast<uint2 *>(tile + (size_t)cc * 4 * tw + 32);
+    uint2 *tab = reinterpret_cast<uint2 *>(tile + (((size_t)cc * tw + 3) & ~(size_t)3));
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int t0 = blockIdx.x * IC_TILE;
     const int grp = blockIdx.y * IC_WARPS + warp;
     const bool live = grp < a.ngroups;
     const float *fb = a.fb + (size_t)blockIdx.z * (size_t)a.fb_stride_dm;
-    const int rows = tw + 3;                 // input samples staged per chunk
+    const int rows = tw;                     // input samples staged per chunk
     const int rstep = (32 * IC_WARPS) / quads;
     const int r0 = tid / quads, q = tid % quads;
 
-    float acc[IC_GROUP][8];
+    float acc[IC_GROUP][8];  // trial k of the group, output sample t0 + lane + 32 i
 #pragma unroll
     for (int k = 0; k < IC_GROUP; ++k)
 #pragma unroll
@@ -137,28 +136,36 @@ __global__ void __launch_bounds__(32 * IC_WARPS, 2) k_incoherent(const IcArgs a)
 
     for (int c0 = 0; c0 < a.nch; c0 += cc) {
         __syncthreads();  // the previous chunk has been consumed
-        // ---- stage: tile copy j of channel c holds fb[t0 + i + j][c0 + c] at index i
-        for (int i = r0; i < rows; i += rstep) {
-            const int t = t0 + i;
-            float gq[4] = {0.f, 0.f, 0.f, 0.f};
-            if (t < a.nt_in) {
-                const float *src = fb + (size_t)t * a.nch + c0 + 4 * q;
-                if (a.vec_in && c0 + 4 * q + 3 < a.nch) {
-                    const float4 w = __ldg(reinterpret_cast<const float4 *>(src));
-                    gq[0] = w.x; gq[1] = w.y; gq[2] = w.z; gq[3] = w.w;
-                } else {
+        // ---- stage the transposed tile: tile[c][i] = fb[t0 + i][c0 + c]; four rows per thread in
+        //      flight (the loads of a batch are issued before its stores); tw = 1 mod 32 keeps the
+        //      transposing stores of a warp (8 channel quads x 4 rows) on 32 different banks
+        for (int ib = r0; ib < rows; ib += 4 * rstep) {
+            float gq[4][4];
 #pragma unroll
-                    for (int e = 0; e < 4; ++e)
-                        if (c0 + 4 * q + e < a.nch) gq[e] = __ldg(src + e);
+            for (int u = 0; u < 4; ++u) {
+                const int i = ib + u * rstep, t = t0 + i;
+#pragma unroll
+                for (int e = 0; e < 4; ++e) gq[u][e] = 0.f;
+                if (i < rows && t < a.nt_in) {
+                    const float *src = fb + (size_t)t * a.nch + c0 + 4 * q;
+                    if (a.vec_in && c0 + 4 * q + 3 < a.nch) {
+                        const float4 w = __ldg(reinterpret_cast<const float4 *>(src));
+                        gq[u][0] = w.x; gq[u][1] = w.y; gq[u][2] = w.z; gq[u][3] = w.w;
+                    } else {
+#pragma unroll
+                        for (int e = 0; e < 4; ++e)
+                            if (c0 + 4 * q + e < a.nch) gq[u][e] = __ldg(src + e);
+                    }
                 }
             }
 #pragma unroll
-            for (int e = 0; e < 4; ++e)
+            for (int u = 0; u < 4; ++u) {
+                const int i = ib + u * rstep;
+                if (i < rows) {
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const int idx = i - j;
-                    if (idx >= 0 && idx < tw) tile[(size_t)((4 * q + e) * 4 + j) * tw + 8 * q + idx] = gq[e];
+                    for (int e = 0; e < 4; ++e) tile[(size_t)(4 * q + e) * tw + i] = gq[u][e];
                 }
+            }
         }
         for (int e = tid; e < IC_WARPS * cc; e += 32 * IC_WARPS) {
             const int w = e / cc, c = e % cc;
@@ -169,42 +176,29 @@ __global__ void __launch_bounds__(32 * IC_WARPS, 2) k_incoherent(const IcArgs a)
         }
         __syncthreads();
         if (!live) continue;
-        // ---- accumulate the chunk: two 8-sample windows per channel serve the 16 trials
+        // ---- accumulate the chunk.  Per channel: the window of the group's first trial (8 conflict-free
+        //      LDS.32), then blocks of four trials -- usually no trial of a block moves the shift (one
+        //      test, 32 straight adds); where one does, the window is re-read at the new shift
 #pragma unroll 1
         for (int c = 0; c < cc; ++c) {
             const uint2 e = tab[warp * cc + c];
-            const float *p = tile + (size_t)(c * 4 + (int)(e.x & 3u)) * tw + 8 * (c >> 2) + (e.x & ~3u) + 4 * lane;
-            float v0[8], v1[8];
-            {
-                const float4 x0 = *reinterpret_cast<const float4 *>(p), x1 = *reinterpret_cast<const float4 *>(p + 4);
-                const float4 y0 = *reinterpret_cast<const float4 *>(p + 128), y1 = *reinterpret_cast<const float4 *>(p + 132);
-                v0[0] = x0.x; v0[1] = x0.y; v0[2] = x0.z; v0[3] = x0.w; v0[4] = x1.x; v0[5] = x1.y; v0[6] = x1.z; v0[7] = x1.w;
-                v1[0] = y0.x; v1[1] = y0.y; v1[2] = y0.z; v1[3] = y0.w; v1[4] = y1.x; v1[5] = y1.y; v1[6] = y1.z; v1[7] = y1.w;
-            }
-            if (e.y == 0u) {
-                // every trial of the group has the same shift in this channel (the usual case)
+            const float *p = tile + (size_t)c * tw + e.x + lane;
+            float v[8];
+            ic_window(v, p);
 #pragma unroll
-                for (int k = 0; k < IC_GROUP; ++k)
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        acc[k][i] += v0[i];
-                        acc[k][4 + i] += v1[i];
-                    }
-            } else {
-#pragma unroll
-                for (int k = 0; k < IC_GROUP; ++k) {
-                    if (k > 0) {
-                        const unsigned n = (e.y >> (2 * k)) & 3u;
-                        if (n >= 1u) { ic_slide(v0); ic_slide(v1); }
-                        if (n >= 2u) { ic_slide(v0); ic_slide(v1); }
-                        if (n == 3u) { ic_slide(v0); ic_slide(v1); }
-                    }
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        acc[k][i] += v0[i];
-                        acc[k][4 + i] += v1[i];
+            for (int k = 0; k < IC_GROUP; ++k) {
+                if (k > 0) {
+                    const unsigned n = (e.y >> (2 * k)) & 3u;
+                    // rare: this trial's shift differs from the previous one (written as a loop so that
+                    // the re-read stays a branch instead of eight predicated loads on the common path)
+#pragma unroll 1
+                    for (unsigned once = 0; once < (n ? 1u : 0u); ++once) {
+                        p += n;
+                        ic_window(v, p);
                     }
                 }
+#pragma unroll
+                for (int i = 0; i < 8; ++i) acc[k][i] += v[i];
             }
         }
     }
@@ -216,15 +210,9 @@ __global__ void __launch_bounds__(32 * IC_WARPS, 2) k_incoherent(const IcArgs a)
         if (k >= gi.y) break;
         float *row = out + (size_t)(gi.x + k) * (size_t)a.ts_pitch;
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            const int t = t0 + 128 * h + 4 * lane;
-            if (a.vec_out && t + 3 < a.nt_out) {
-                *reinterpret_cast<float4 *>(row + t) = make_float4(acc[k][4 * h], acc[k][4 * h + 1], acc[k][4 * h + 2], acc[k][4 * h + 3]);
-            } else {
-#pragma unroll
-                for (int i = 0; i < 4; ++i)
-                    if (t + i < a.nt_out) row[t + i] = acc[k][4 * h + i];
-            }
+        for (int i = 0; i < 8; ++i) {
+            const int t = t0 + lane + 32 * i;
+            if (t < a.nt_out) row[t] = acc[k][i];
         }
     }
 }
@@ -248,16 +236,15 @@ cudaError_t launch_incoherent(const Geometry &g, const IncoherentTables &T, cons
     a.fb = d_fb; a.fb_stride_dm = fb_stride_dm; a.ts = d_ts; a.ts_stride_dm = ts_stride_dm; a.ts_pitch = ts_pitch;
     a.entries = d_entries; a.groups = d_groups;
     a.nt_in = (int)nt_in; a.nt_out = (int)nt_out; a.nch = nch; a.ngroups = ngroups;
-    a.tw = ((T.range + 3) & ~3) + IC_TILE + 8;
+    a.tw = ((T.range + IC_TILE + 30) & ~31) + 1;  // >= range + 256 and = 1 mod 32
     a.vec_in = (nch % 4 == 0 && fb_stride_dm % 4 == 0 && (reinterpret_cast<uintptr_t>(d_fb) & 15) == 0) ? 1 : 0;
-    a.vec_out = (ts_pitch % 4 == 0 && ts_stride_dm % 4 == 0 && (reinterpret_cast<uintptr_t>(d_ts) & 15) == 0) ? 1 : 0;
-    // channels per chunk: the largest of 16, 8, 4 whose tile lets two CTAs share an SM, else whatever fits
-    auto smem_for = [&](int cc) { return sizeof(float) * ((size_t)cc * 4 * a.tw + 32) + sizeof(uint2) * IC_WARPS * cc; };
+    // channels per chunk: the largest of 32, 16, 8, 4 whose tile lets two CTAs share an SM, else whatever fits
+    auto smem_for = [&](int cc) { return sizeof(float) * (((size_t)cc * a.tw + 3) & ~(size_t)3) + sizeof(uint2) * IC_WARPS * cc; };
     int cc = 0;
-    for (int c : {16, 8, 4})
-        if (smem_for(c) <= 110 * 1024) { cc = c; break; }
+    for (int c : {32, 16, 8, 4})
+        if (smem_for(c) <= 72 * 1024) { cc = c; break; }
     if (!cc)
-        for (int c : {16, 8, 4})
+        for (int c : {32, 16, 8, 4})
             if (smem_for(c) <= 227 * 1024) { cc = c; break; }
     if (!cc) return cudaErrorInvalidValue;
     a.cc = cc;
