@@ -124,7 +124,7 @@ class Plan:
         self.ndm, self.in_dtype, self.chirp_ref = ndm, in_dtype, chirp_ref
 
     def __del__(self):
-        if getattr(self, "handle", None):
+        if getattr(self, "handle", None) and _lib is not None:   # _lib is None during interpreter shutdown
             _lib.cdmt_plan_destroy(self.handle)
             self.handle = None
 
