@@ -291,3 +291,22 @@ def test_errors_are_codes_not_crashes(cdmt):
     cdmt.cdmt_execute(plan, x, cfg.nsamp, cfg.nsamp, out, out[0].numel(), ws, ws.numel())
     torch.cuda.synchronize()
     assert float(out.abs().max()) == 0.0
+
+
+# ---------------------------------------------------------------- repeatability (stands in for racecheck)
+@pytest.mark.parametrize("kern", [3, 5, 4])
+def test_fused_kernels_are_bit_reproducible(cdmt, kern):
+    """compute-sanitizer's racecheck is not available on the GPU pool.  The fused kernels exchange data
+    through shared memory under split mbarriers; a missing wait would show as run-to-run differences.
+    Twenty executes of the same plan on the same input (a grid of several waves, every DM trial written
+    into its own plane) must be bit-identical."""
+    cfg = synth.small_config(nsub=24, nsamp=2 ** 18, nfft=65536, noverlap=16384, nchan=16, ndec=16,
+                             dm=tuple(np.arange(24) * 1.25), f_lo=119.0)
+    x = synth.generate(cfg)
+    plan = cdmt.cdmt_plan_create(**cfg.plan_kwargs())
+    cdmt.cdmt_plan_set_option(plan, cdmt.OPT_FUSED_KERNEL, kern)
+    d_in = torch.from_numpy(x).cuda()
+    first = cdmt.run_on_device(plan, d_in, cfg.nsamp).clone()
+    for _ in range(20):
+        again = cdmt.run_on_device(plan, d_in, cfg.nsamp)
+        assert torch.equal(first, again)
