@@ -111,6 +111,49 @@ __device__ __forceinline__ void ic_window(float (&v)[8], const float *p)
     for (int i = 0; i < 8; ++i) v[i] = p[32 * i];
 }
 
+// Trial K of the group: if its 2-bit field of `ey` is non-zero, advance the shared-memory address by
+// that many samples and re-read the window.  Written in PTX so that the test is one predicate-setting
+// logic instruction and the branch is declared warp-uniform (`bra.uni`: every lane holds the same
+// table word) -- no reconvergence bookkeeping, nothing but two instructions on the common path.
+template <int K>
+__device__ __forceinline__ void ic_step(float (&v)[8], unsigned &sp, unsigned ey)
+{
+    asm volatile(
+        "{\n\t"
+        ".reg .pred q;\n\t"
+        ".reg .b32 t;\n\t"
+        "and.b32 t, %9, %10;\n\t"
+        "setp.eq.u32 q, t, 0;\n\t"
+        "@q bra.uni IC_SKIP;\n\t"
+        "shr.u32 t, t, %11;\n\t"
+        "shl.b32 t, t, 2;\n\t"
+        "add.u32 %8, %8, t;\n\t"
+        "ld.shared.f32 %0, [%8];\n\t"
+        "ld.shared.f32 %1, [%8+128];\n\t"
+        "ld.shared.f32 %2, [%8+256];\n\t"
+        "ld.shared.f32 %3, [%8+384];\n\t"
+        "ld.shared.f32 %4, [%8+512];\n\t"
+        "ld.shared.f32 %5, [%8+640];\n\t"
+        "ld.shared.f32 %6, [%8+768];\n\t"
+        "ld.shared.f32 %7, [%8+896];\n\t"
+        "IC_SKIP:\n\t"
+        "}"
+        : "+f"(v[0]), "+f"(v[1]), "+f"(v[2]), "+f"(v[3]), "+f"(v[4]), "+f"(v[5]), "+f"(v[6]), "+f"(v[7]), "+r"(sp)
+        : "r"(ey), "n"(3u << (2 * K)), "n"(2 * K)
+        : "memory");
+}
+
+template <int K>
+__device__ __forceinline__ void ic_trials(float (&acc)[IC_GROUP][8], float (&v)[8], unsigned &sp, unsigned ey)
+{
+    if constexpr (K < IC_GROUP) {
+        if constexpr (K > 0) ic_step<K>(v, sp, ey);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) acc[K][i] += v[i];
+        ic_trials<K + 1>(acc, v, sp, ey);
+    }
+}
+
 // grid (ceil(nt_out / 256), ceil(ngroups / 4), ndm), 128 threads; dynamic shared memory:
 // float tile[cc][tw] and uint2 tab[4][cc]
 __global__ void __launch_bounds__(32 * IC_WARPS, 3) k_incoherent(const IcArgs a)
@@ -185,21 +228,8 @@ __global__ void __launch_bounds__(32 * IC_WARPS, 3) k_incoherent(const IcArgs a)
             const float *p = tile + (size_t)c * tw + e.x + lane;
             float v[8];
             ic_window(v, p);
-#pragma unroll
-            for (int k = 0; k < IC_GROUP; ++k) {
-                if (k > 0) {
-                    const unsigned n = (e.y >> (2 * k)) & 3u;
-                    // rare: this trial's shift differs from the previous one (written as a loop so that
-                    // the re-read stays a branch instead of eight predicated loads on the common path)
-#pragma unroll 1
-                    for (unsigned once = 0; once < (n ? 1u : 0u); ++once) {
-                        p += n;
-                        ic_window(v, p);
-                    }
-                }
-#pragma unroll
-                for (int i = 0; i < 8; ++i) acc[k][i] += v[i];
-            }
+            unsigned sp = (unsigned)__cvta_generic_to_shared(p);
+            ic_trials<0>(acc, v, sp, e.y);
         }
     }
     if (!live) return;
