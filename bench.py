@@ -60,6 +60,23 @@ def rank_workload(cfg: synth.Config, rank: int, world: int) -> synth.Config:
     return cfg
 
 
+def subband_range(nsub: int, rank: int, world: int):
+    """Strong scaling (--shard subband; PAPER.md:137 runs subband groups on separate GPUs): rank r
+    owns the contiguous subbands [s0, s1) of the ONE observation; no exchange step, outputs concatenate."""
+    return (nsub * rank) // world, (nsub * (rank + 1)) // world
+
+
+def rank_piece(cfg: synth.Config, rank: int, world: int, shard: str):
+    """(config of this rank's plan, first global subband it generates)."""
+    if shard == "subband" and world > 1:
+        import dataclasses
+        s0, s1 = subband_range(cfg.nsub, rank, world)
+        if s1 <= s0:
+            raise SystemExit("--shard subband needs at least one subband per rank")
+        return dataclasses.replace(cfg, nsub=s1 - s0, fcen_mhz=cfg.fcen_mhz[s0:s1]), s0
+    return rank_workload(cfg, rank, world), 0
+
+
 def max_over_ranks(value: float, world: int, device=None) -> float:
     """MAX all-reduce of a per-rank scalar (device time); identity for one rank."""
     if world <= 1:
@@ -183,7 +200,9 @@ def workload_config(cfg, args):
                cfg.ndm, "int8" if cfg.in_dtype == synth.IN_CI8 else "complex64"),
             "nsub": cfg.nsub, "nsamp": cfg.nsamp, "nfft": cfg.nfft, "noverlap": cfg.noverlap,
             "nchan": cfg.nchan, "ndec": cfg.ndec, "ndm": cfg.ndm, "nblock": cfg.nblock,
-            "parallelism": "replicas x%d (one observation per GPU, no collective)" % args.gpus,
+            "parallelism": ("subbands of one observation split over %d GPUs (no collective)" % args.gpus)
+                           if getattr(args, "shard", "replicas") == "subband" and args.gpus > 1 else
+                           "replicas x%d (one observation per GPU, no collective)" % args.gpus,
             "l2": "inputs (%.1f GB) and spectra exceed the 126 MB L2; no flush needed" % (
                 cfg.nsub * 2 * cfg.nsamp * (2 if cfg.in_dtype == synth.IN_CI8 else 8) / 1e9)}
 
@@ -201,6 +220,9 @@ def main():
     ap.add_argument("--dm-tile", type=int, default=0)
     ap.add_argument("--fused-kernel", type=int, default=0, help="CDMT_OPT_FUSED_KERNEL (0 = library default)")
     ap.add_argument("--gen-threads", type=int, default=0)
+    ap.add_argument("--shard", default="replicas", choices=["replicas", "subband"],
+                    help="N > 1: one observation per GPU (weak scaling, default) or the subbands of one "
+                         "observation split over the GPUs (strong scaling); neither has a collective")
     ap.add_argument("--no-redigitize", action="store_true", help="skip the extra cdmt_redigitize timing (N1)")
     ap.add_argument("--no-incoherent", action="store_true", help="skip the extra cdmt_incoherent_dedisperse timing (N2)")
     ap.add_argument("--fine-step", type=float, default=0.002, help="fine DM step of the incoherent leg (PAPER.md:141)")
@@ -209,11 +231,14 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
-    cfg = rank_workload(synth.make_config(args.config), rank, world)
-
+    full_cfg = synth.make_config(args.config)
     if args.impl == "reference":
+        cfg = rank_workload(full_cfg, rank, world)
         run_reference(args, cfg, rank, world)
         return
+    cfg, sub0 = rank_piece(full_cfg, rank, world, args.shard)
+    gen_cfg = full_cfg if args.shard == "subband" and world > 1 else cfg   # generator sees global subband indices
+    strong = args.shard == "subband" and world > 1
 
     import torch
     import torch.distributed as dist
@@ -246,7 +271,7 @@ def main():
     from concurrent.futures import ThreadPoolExecutor
     t_gen = time.perf_counter()
     with ThreadPoolExecutor(nthreads) as ex:
-        for s, xs in zip(range(cfg.nsub), ex.map(lambda s: synth.generate_subband(cfg, s), range(cfg.nsub))):
+        for s, xs in zip(range(cfg.nsub), ex.map(lambda s: synth.generate_subband(gen_cfg, sub0 + s), range(cfg.nsub))):
             if s == 0:
                 x_sub0 = xs
             t = torch.from_numpy(xs)
@@ -321,7 +346,8 @@ def main():
     ms = max_over_ranks(ms, world, dev)
     sec_per_step = ms * 1e-3 / args.steps
     samples_dm = float(cfg.nsub) * cfg.nsamp * cfg.ndm
-    value = whole_job_value(cfg, world, sec_per_step)
+    # weak: every rank processed a whole observation; strong: the ranks share one
+    value = whole_job_value(full_cfg, 1, sec_per_step) if strong else whole_job_value(cfg, world, sec_per_step)
 
     # ---- roofline of the dominant kernel (fused per-DM kernel): ALU bound
     units_per_step = cfg.nsub * nb_total
@@ -431,7 +457,7 @@ def main():
         dt = (time.perf_counter() - t0) / ksteps
         dt = max_over_ranks(dt, world, dev)
         h2d_b, d2h_b = cdmt.cdmt_host_traffic_bytes(plan, cfg.nsamp)
-        e2e = {"value": whole_job_value(cfg, world, dt), "unit": UNIT,
+        e2e = {"value": whole_job_value(full_cfg, 1, dt) if strong else whole_job_value(cfg, world, dt), "unit": UNIT,
                "h2d_bytes_per_step": int(h2d_b), "d2h_bytes_per_step": int(d2h_b),
                "ms_per_step": dt * 1e3, "steps": ksteps,
                "api": "cdmt_execute_host (pinned host in/out, double-buffered copy streams)"}
@@ -453,8 +479,8 @@ def main():
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": sec_per_step * 1e3, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": workload_config(cfg, args),
+            "scaling": "strong" if strong else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": workload_config(full_cfg if strong else cfg, args),
             "real_time_factor": cfg.nsamp * synth.TSAMP_S / sec_per_step,
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
             "roofline": roofline, "cpu_baseline": cpu, "redigitize": redig, "incoherent": incoh,

@@ -76,7 +76,7 @@ enum {
  *   bw_mhz    subband bandwidth = complex sample rate, MHz (> 0; fcen - bw/2 > 0)
  *   nfft      N_bin, power of two, 256 <= nfft <= 2^20
  *   noverlap  n_d n_c in INPUT samples: 0 <= noverlap < nfft, noverlap % (2 nchan) == 0
- *   nchan     n_c, power of two, 16 <= nfft/nchan <= 16384
+ *   nchan     n_c, power of two, 16 <= nfft/nchan <= 8192
  *   ndec      time-integration factor >= 1, (nfft - noverlap) % (nchan ndec) == 0
  *   ndm, dm   HOST [ndm] DM trials in pc cm^-3 (any sign: -DM applies the conjugate chirp); copied
  *   in_dtype  CDMT_IN_*; chirp_ref CDMT_REF_*
@@ -229,6 +229,18 @@ double cdmt_sweep_seconds(double fcen_mhz, double bw_mhz, double dm);
  * that covers the sweep of the lowest channel (REF_CHANNEL) or lowest subband (REF_SUBBAND)
  * at the largest |DM| of the plan. */
 long long cdmt_min_overlap(const cdmt_plan *plan);
+
+/* Sizes from the dispersion sweep ("n_d n_c >= r t_d ... for the channel with the lowest
+ * frequency"; PAPER.md:175 names the single N_bin / n_d for all subbands as an
+ * inefficiency): for the given subbands (call it per subband, or per group of subbands that share a
+ * plan) returns the smallest legal noverlap (input samples; a multiple of 2 nchan and of nchan ndec)
+ * that covers the sweep of the lowest channel (REF_CHANNEL) or subband (REF_SUBBAND) at DM
+ * dm_max_abs, and the smallest power-of-two nfft this library supports whose kept fraction
+ * (nfft - noverlap) / nfft is at least min_efficiency (0 < min_efficiency < 1).  Host arithmetic only.
+ * Errors: CDMT_ERR_ARG, CDMT_ERR_SIZE (no supported nfft reaches the efficiency). */
+int cdmt_suggest_sizes(int nsub, const double *fcen_mhz, double bw_mhz, int nchan, int ndec,
+                       double dm_max_abs, int chirp_ref, double min_efficiency, int *nfft,
+                       int *noverlap);
 
 /* Measure the FP32 FMA rate of the device the stream belongs to (the "alu" roofline
  * denominator): runs `iters` dependent-chain FMA launches and returns

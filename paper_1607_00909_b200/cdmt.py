@@ -28,7 +28,7 @@ EXPORTS = [
     "cdmt_execute", "cdmt_execute_host", "cdmt_host_scratch_bytes", "cdmt_host_traffic_bytes", "cdmt_unpack",
     "cdmt_forward_spectrum", "cdmt_redigitize", "cdmt_redigitize_workspace_bytes",
     "cdmt_incoherent_query", "cdmt_incoherent_shifts", "cdmt_incoherent_dedisperse",
-    "cdmt_sweep_seconds", "cdmt_min_overlap",
+    "cdmt_sweep_seconds", "cdmt_min_overlap", "cdmt_suggest_sizes",
     "cdmt_measure_fp32_peak", "cdmt_last_launch_count", "cdmt_profile_read", "cdmt_strerror",
     "cdmt_version",
 ]
@@ -61,6 +61,7 @@ _lib.cdmt_incoherent_shifts.argtypes = [_vp, _i, C.POINTER(_d), _vp]
 _lib.cdmt_incoherent_dedisperse.argtypes = [_vp, _vp, _ll, _ll, _i, C.POINTER(_d), _vp, _ll, _ll, _vp, _sz, _vp]
 _lib.cdmt_sweep_seconds.argtypes = [_d, _d, _d]
 _lib.cdmt_sweep_seconds.restype = _d
+_lib.cdmt_suggest_sizes.argtypes = [_i, C.POINTER(_d), _d, _i, _i, _d, _i, _d, C.POINTER(_i), C.POINTER(_i)]
 _lib.cdmt_min_overlap.argtypes = [_vp]
 _lib.cdmt_min_overlap.restype = _ll
 _lib.cdmt_measure_fp32_peak.argtypes = [_vp, _sz, _i, C.POINTER(_d), _vp]
@@ -247,6 +248,17 @@ def cdmt_incoherent_dedisperse(plan: Plan, d_fb, fb_stride_dm: int, nt_in: int, 
 
 def cdmt_min_overlap(plan: Plan) -> int:
     return _lib.cdmt_min_overlap(plan.handle)
+
+
+def cdmt_suggest_sizes(fcen_mhz, bw_mhz: float, nchan: int, ndec: int, dm_max_abs: float,
+                       chirp_ref: int = REF_CHANNEL, min_efficiency: float = 0.75):
+    """(nfft, noverlap) from the dispersion sweep of the lowest channel / subband."""
+    f = np.ascontiguousarray(fcen_mhz, dtype=np.float64).reshape(-1)
+    nfft, nov = _i(), _i()
+    _check(_lib.cdmt_suggest_sizes(f.size, f.ctypes.data_as(C.POINTER(_d)), float(bw_mhz), int(nchan), int(ndec),
+                                   float(dm_max_abs), int(chirp_ref), float(min_efficiency), C.byref(nfft),
+                                   C.byref(nov)), "cdmt_suggest_sizes")
+    return nfft.value, nov.value
 
 
 def cdmt_last_launch_count(plan: Plan) -> int:

@@ -647,6 +647,50 @@ extern "C" long long cdmt_min_overlap(const cdmt_plan *plan)
     return (samples + q - 1) / q * q;
 }
 
+// N_bin and n_d follow from the dispersion sweep (Eq. 2) of the lowest channel
+// at the largest DM; the paper fixes one pair for all subbands and names that as an inefficiency.
+extern "C" int cdmt_suggest_sizes(int nsub, const double *fcen_mhz, double bw_mhz, int nchan, int ndec,
+                                  double dm_max_abs, int chirp_ref, double min_efficiency, int *nfft, int *noverlap)
+{
+    if (!fcen_mhz || !nfft || !noverlap || nsub < 1) return CDMT_ERR_ARG;
+    if (!(bw_mhz > 0.0) || !std::isfinite(bw_mhz) || !std::isfinite(dm_max_abs) || dm_max_abs < 0.0) return CDMT_ERR_ARG;
+    if (!(min_efficiency > 0.0) || !(min_efficiency < 1.0)) return CDMT_ERR_ARG;
+    if (chirp_ref != CDMT_REF_CHANNEL && chirp_ref != CDMT_REF_SUBBAND) return CDMT_ERR_ARG;
+    if (!is_pow2(nchan) || ndec < 1) return CDMT_ERR_SIZE;
+    double fmin = fcen_mhz[0];
+    for (int s = 0; s < nsub; ++s) {
+        if (!std::isfinite(fcen_mhz[s]) || !(fcen_mhz[s] - 0.5 * bw_mhz > 0.0)) return CDMT_ERR_ARG;
+        fmin = fcen_mhz[s] < fmin ? fcen_mhz[s] : fmin;
+    }
+    double td;
+    if (chirp_ref == CDMT_REF_CHANNEL) {
+        const double cw = bw_mhz / nchan;
+        td = cdmt_sweep_seconds(fmin - 0.5 * bw_mhz + 0.5 * cw, cw, dm_max_abs);
+    } else {
+        td = cdmt_sweep_seconds(fmin, bw_mhz, dm_max_abs);
+    }
+    const long long sweep = (long long)std::ceil(td * bw_mhz * 1e6);   // input samples (r t_d)
+    // noverlap: multiple of 2 nchan (half per edge, whole channelised samples) and of nchan ndec
+    long long q = 2LL * nchan, r = (long long)nchan * ndec;
+    long long a = q, b = r;
+    while (b) { const long long t = a % b; a = b; b = t; }
+    const long long unit = q / a * r;
+    const long long ov = (sweep + unit - 1) / unit * unit;
+    // nfft: smallest power of two whose kept fraction reaches min_efficiency and that the kernels support
+    for (long long n = 256; n <= (1LL << 20); n <<= 1) {
+        if (n % nchan || !fused_len_supported((int)(n / nchan))) continue;
+        if (n % r) continue;
+        if (ov >= n) continue;
+        if ((double)(n - ov) < min_efficiency * (double)n) continue;
+        const int lg = ilog2(n);
+        if (!forward_len_supported(1 << ((lg + 1) / 2)) || !forward_len_supported((int)(n >> ((lg + 1) / 2)))) continue;
+        *nfft = (int)n;
+        *noverlap = (int)ov;
+        return CDMT_OK;
+    }
+    return CDMT_ERR_SIZE;
+}
+
 extern "C" long long cdmt_last_launch_count(const cdmt_plan *plan) { return plan ? plan->last_launches : -1; }
 
 extern "C" int cdmt_measure_fp32_peak(void *d_scratch, size_t scratch_bytes, int iters, double *tflops,

@@ -196,3 +196,45 @@ def test_product_path_does_not_import_the_oracle():
             txt = open(os.path.join(ROOT, "oracle", f)).read()
             assert not re.search(r"^\s*(from|import)\s+paper_1607_00909_b200", txt, flags=re.M), f
             assert "libcdmt" not in txt and "csrc" not in txt.replace("paper_1607_00909_b200/csrc/", ""), f
+
+
+def test_suggest_sizes_follow_eq2_and_are_legal(cdmt):
+    """cdmt_suggest_sizes: noverlap covers r t_d of the lowest channel at the largest
+    DM (Eq. 2 via the oracle's separately written sweep), is legal for cdmt_plan_create, nfft keeps the
+    requested fraction; higher subbands and lower DMs get smaller sizes (the paper's own inefficiency)."""
+    from oracle import cdmt_oracle as orc
+    bw, nchan = 0.1953125, 8
+    lo = np.array([114.93 + bw / 2])                      # the paper's lowest survey subband (PAPER.md:167)
+    nfft, nov = cdmt.cdmt_suggest_sizes(lo, bw, nchan, 1, 79.5)
+    cw = bw / nchan
+    need = orc.sweep_seconds(lo[0] - bw / 2 + cw / 2, cw, 79.5) * bw * 1e6
+    assert 2071 < need < 2073                              # PAPER.md:71 / SURVEY: r t_d = 2072 input samples
+    assert need <= nov < need + 2 * nchan and nov % (2 * nchan) == 0
+    assert (nfft - nov) >= 0.75 * nfft and (nfft // 2 - nov) < 0.75 * (nfft // 2)
+    assert (nfft, nov) == (16384, 2080)                    # against the paper's fixed 65536 / 16384 (PAPER.md:139)
+    plan = cdmt.cdmt_plan_create(nsub=1, fcen_mhz=lo, bw_mhz=bw, nfft=nfft, noverlap=nov, nchan=nchan, ndec=1,
+                                 dm=[0.0, 79.5])
+    assert cdmt.cdmt_min_overlap(plan) == nov
+    # per-subband sizes: the top of the LOFAR band needs a quarter of the overlap
+    hi = np.array([175.0])
+    nfft_hi, nov_hi = cdmt.cdmt_suggest_sizes(hi, bw, nchan, 1, 79.5)
+    assert nov_hi < nov / 3 and nfft_hi <= nfft
+    # monotone in DM, ndec divisibility, efficiency knob
+    prev = 0
+    for dm in (1.0, 10.0, 40.0, 79.5):
+        n, o = cdmt.cdmt_suggest_sizes(lo, bw, 16, 16, dm)
+        assert o >= prev and o % (16 * 16) == 0 and (n - o) % (16 * 16) == 0
+        prev = o
+    n9, o9 = cdmt.cdmt_suggest_sizes(lo, bw, nchan, 1, 79.5, min_efficiency=0.9)
+    assert o9 == nov and n9 > nfft and (n9 - o9) >= 0.9 * n9
+    # subband-referenced chirp: the sweep of the whole subband; no supported nfft at 8 channels -> status
+    with pytest.raises(cdmt.CdmtError) as e:
+        cdmt.cdmt_suggest_sizes(lo, bw, nchan, 1, 79.5, cdmt.REF_SUBBAND)
+    assert e.value.status == cdmt.ERR_SIZE
+    n32, o32 = cdmt.cdmt_suggest_sizes(lo, bw, 32, 1, 79.5, cdmt.REF_SUBBAND, 0.5)
+    assert o32 >= orc.sweep_seconds(lo[0], bw, 79.5) * bw * 1e6 and n32 // 32 <= 8192
+    for bad in (dict(min_efficiency=1.0), dict(min_efficiency=0.0), dict(dm_max_abs=-1.0)):
+        kw = dict(fcen_mhz=lo, bw_mhz=bw, nchan=nchan, ndec=1, dm_max_abs=79.5)
+        kw.update(bad)
+        with pytest.raises(cdmt.CdmtError):
+            cdmt.cdmt_suggest_sizes(**kw)

@@ -86,3 +86,28 @@ def test_reference_arm_two_ranks_prints_one_line():
     assert d["impl"] == "reference" and d["metric"] == bench.METRIC and d["value"] > 0
     assert d["cpu_baseline"]["kind"] == "oracle" and d["e2e"]["h2d_bytes_per_step"] == 0
     assert d["n_gpus"] == 2 and d["higher_is_better"] is True
+
+
+def test_subband_sharding_partitions_the_observation():
+    """--shard subband (strong scaling): the ranks' subband ranges tile [0, nsub) without
+    overlap, each rank's plan sees its own centre frequencies, and the generator is indexed by the
+    GLOBAL subband so that the pieces are the pieces of the one observation."""
+    c3 = synth.make_config("c3")
+    for world in (1, 2, 3, 8):
+        rng = [bench.subband_range(c3.nsub, r, world) for r in range(world)]
+        assert rng[0][0] == 0 and rng[-1][1] == c3.nsub
+        assert all(rng[i][1] == rng[i + 1][0] for i in range(world - 1))
+        assert max(b - a for a, b in rng) - min(b - a for a, b in rng) <= 1
+    piece, s0 = bench.rank_piece(synth.make_config("c3"), 3, 8, "subband")
+    assert piece.nsub == 36 and s0 == 108 and np.array_equal(piece.fcen_mhz, c3.fcen_mhz[108:144])
+    assert piece.nblock == c3.nblock and piece.ndm == c3.ndm and piece.seed == c3.seed
+    solo, s0 = bench.rank_piece(synth.make_config("c3"), 0, 1, "subband")
+    assert solo.nsub == c3.nsub and s0 == 0
+    rep, s0 = bench.rank_piece(synth.make_config("c1"), 1, 2, "replicas")
+    assert rep.nsub == 1 and s0 == 0 and rep.seed != synth.make_config("c1").seed
+    # a piece's data equals the slice of the whole observation
+    small = synth.small_config(nsub=4, nsamp=2 ** 13, nfft=4096, noverlap=1024, nchan=8, ndec=4, dm=(0.0, 3.0))
+    whole = synth.generate(small)
+    pc, s0 = bench.rank_piece(small, 1, 2, "subband")
+    got = np.stack([synth.generate_subband(small, s0 + s) for s in range(pc.nsub)])
+    assert np.array_equal(got, whole[2:4])
