@@ -207,7 +207,7 @@ int cdmt_redigitize_workspace_bytes(const cdmt_plan *plan, long long nblock, siz
  *                  nt_out samples per row (ts_pitch >= nt_out, ts_stride_dm >= nfine * ts_pitch)
  *   d_workspace    DEVICE scratch, 256-byte aligned, >= workspace_bytes from cdmt_incoherent_query
  * cdmt_incoherent_query: host arithmetic only; any output pointer may be NULL.  ngroups = number
- * of trial groups the kernel works in (<= 16 trials each; fewer where the shifts of consecutive
+ * of trial groups the kernel works in (<= 8 trials each; fewer where the shifts of consecutive
  * trials differ by more than the kernel's register window allows).
  * cdmt_incoherent_shifts: copies the shift table [nfine][nsub*nchan] to HOST memory.
  * Sums are accumulated in float32 in channel order.

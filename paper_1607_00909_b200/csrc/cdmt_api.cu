@@ -619,7 +619,7 @@ extern "C" int cdmt_incoherent_dedisperse(cdmt_plan *plan, const float *d_fb, lo
     const long long nt_out = nt_in - plan->ic.range;
     if (nt_in < 1 || nt_in > (1LL << 30) || nt_out < 1) return CDMT_ERR_SIZE;
     if (fb_stride_dm < nt_in * nch || ts_pitch < nt_out || ts_stride_dm < (long long)nfine * ts_pitch) return CDMT_ERR_SIZE;
-    if (g.ndm > 65535 || (plan->ic.groups.size() + 3) / 4 > 65535) return CDMT_ERR_SIZE;
+    if (g.ndm > 65535 || plan->ic.groups.size() / 4 > 65535) return CDMT_ERR_SIZE;
     if (workspace_bytes < incoherent_workspace_bytes(plan->ic)) return CDMT_ERR_WORKSPACE;
     plan->last_launches = 0;
     return check_cuda(launch_incoherent(g, plan->ic, d_fb, fb_stride_dm, nt_in, d_ts, ts_stride_dm, ts_pitch,

@@ -7,13 +7,13 @@
 //   ts[d][k][t] = sum_j fb[d][t + shift[k][j] - smin][j],  t < nt - (smax - smin)
 //
 // The filterbank is time-major, channel-fastest; dedispersion wants runs along time.
-// A CTA (4 warps) owns 256 output samples of 64 trials: it walks the channels in chunks of CC,
+// A CTA (8 warps) owns 256 output samples of 64 trials: it walks the channels in chunks of CC,
 // transposing each chunk's tile [CC][256 + range] into shared memory (coalesced loads along
-// channels), and every warp adds the chunk into the 16 trials x 8 samples (t = lane + 32 i) it
-// keeps in registers.  The host orders the trials by DM offset and cuts them into groups of 16, so
+// channels), and every warp adds the chunk into the 8 trials x 8 samples (t = lane + 32 i) it
+// keeps in registers.  The host orders the trials by DM offset and cuts them into groups of 8, so
 // inside a group the shift of a channel only grows, and by little: per channel a thread reads its 8
 // samples at the first trial's shift (conflict-free LDS.32) and re-reads them only where a trial's
-// shift differs from the previous one (2-bit increments per trial from a table).  128 FADD per 8-24
+// shift differs from the previous one (2-bit increments per trial from a table).  64 FADD per 8-16
 // floats read from shared memory: the kernel is bound by the FP32 pipe (4 adds per float read would
 // be the break-even with shared-memory bandwidth).
 #include <algorithm>
@@ -25,8 +25,8 @@
 namespace cdmt {
 
 constexpr int IC_TILE = 256;     // output samples per CTA
-constexpr int IC_GROUP = 16;     // trials per warp
-constexpr int IC_WARPS = 4;      // warps (trial groups) per CTA
+constexpr int IC_GROUP = 8;      // trials per warp (measured on c3: 16 x 4 warps 85 ms, 8 x 8 warps 72 ms, 4 x 8 warps 74 ms)
+constexpr int IC_WARPS = 8;      // warps (trial groups) per CTA
 constexpr int IC_MAXSTEP = 3;    // largest growth of a channel's shift from one trial to the next (2-bit table field)
 
 // ------------------------------------------------------------------------------------------ host
@@ -56,7 +56,7 @@ bool incoherent_plan(const Geometry &g, const double *h_fcen, int nfine, const d
         }
     T->smin = smin;
     T->range = smax - smin;
-    // groups of up to 16 consecutive trials whose shifts grow by at most 3 samples per trial
+    // groups of up to IC_GROUP consecutive trials whose shifts grow by at most 3 samples per trial
     T->groups.clear();
     T->entries.clear();
     int k0 = 0;
@@ -154,9 +154,9 @@ __device__ __forceinline__ void ic_trials(float (&acc)[IC_GROUP][8], float (&v)[
     }
 }
 
-// grid (ceil(nt_out / 256), ceil(ngroups / 4), ndm), 128 threads; dynamic shared memory:
-// float tile[cc][tw] and uint2 tab[4][cc]
-__global__ void __launch_bounds__(32 * IC_WARPS, 3) k_incoherent(const IcArgs a)
+// grid (ceil(nt_out / 256), ceil(ngroups / IC_WARPS), ndm), 32 IC_WARPS threads; dynamic shared memory:
+// float tile[cc][tw] and uint2 tab[IC_WARPS][cc]
+__global__ void __launch_bounds__(32 * IC_WARPS, 2) k_incoherent(const IcArgs a)
 {
     extern __shared__ float4 ic_smem4[];
     float *tile = reinterpret_cast<float *>(ic_smem4);
@@ -229,7 +229,8 @@ __global__ void __launch_bounds__(32 * IC_WARPS, 3) k_incoherent(const IcArgs a)
             float v[8];
             ic_window(v, p);
             unsigned sp = (unsigned)__cvta_generic_to_shared(p);
-            ic_trials<0>(acc, v, sp, e.y);
+            // the table word is the same in every lane; the shuffle lets the compiler know it
+            ic_trials<0>(acc, v, sp, __shfl_sync(0xffffffffu, e.y, 0));
         }
     }
     if (!live) return;
