@@ -141,14 +141,14 @@ __global__ void __launch_bounds__(L) k_fwd_pass(const void *__restrict__ src_v, 
     if (MODE == 0) {
         const int unit = unit0 + (row >> 1), b = unit / nsub, s = unit % nsub;
         const size_t src0 = (size_t)(2 * s + p) * (size_t)in_stride_pol + (size_t)b * step + (size_t)tile * FWD_BATCH;
-#pragma unroll 4
+#pragma unroll 16  // all 16 loads of a thread in flight (HBM latency; measured 11.8 -> 9.6 ms per c3 step)
         for (int e = tid; e < L * FWD_BATCH; e += NT) {
             const int n1i = e / FWD_BATCH, col = e % FWD_BATCH;
             smem[Addr::at(n1i, col)] = load_sample<IN>(src_v, src0 + (size_t)n1i * n2 + col);
         }
     } else {
         const float2 *src = reinterpret_cast<const float2 *>(src_v) + plane + (size_t)tile * FWD_BATCH * n2;
-#pragma unroll 4
+#pragma unroll 16
         for (int e = tid; e < L * FWD_BATCH; e += NT) {
             const int rr = e / L, n2i = e % L;
             smem[Addr::at(n2i, rr)] = __ldg(src + (size_t)rr * n2 + n2i);
