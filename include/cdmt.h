@@ -210,7 +210,10 @@ int cdmt_redigitize_workspace_bytes(const cdmt_plan *plan, long long nblock, siz
  * of trial groups the kernel works in (<= 8 trials each; fewer where the shifts of consecutive
  * trials differ by more than the kernel's register window allows).
  * cdmt_incoherent_shifts: copies the shift table [nfine][nsub*nchan] to HOST memory.
- * Sums are accumulated in float32 in channel order.
+ * Sums are accumulated in float32 in channel order.  The plan caches the shift and group tables of the
+ * last ddm list it was given (these three calls therefore take a non-const plan and, like every other
+ * call, must not run concurrently on one plan); cdmt_incoherent_dedisperse uploads them with
+ * cudaMemcpyAsync from pageable host memory on `cuda_stream` and queues one kernel.
  * Errors: CDMT_ERR_ARG (null / misaligned pointer, non-finite or non-ascending ddm), CDMT_ERR_SIZE
  * (nt_in <= shift_range, short strides), CDMT_ERR_WORKSPACE, CDMT_ERR_ALLOC, CDMT_ERR_CUDA.
  */
