@@ -220,6 +220,8 @@ def main():
     ap.add_argument("--dm-tile", type=int, default=0)
     ap.add_argument("--fused-kernel", type=int, default=0, help="CDMT_OPT_FUSED_KERNEL (0 = library default)")
     ap.add_argument("--gen-threads", type=int, default=0)
+    ap.add_argument("--host-group-blocks", type=int, default=0,
+                    help="CDMT_OPT_HOST_GROUP_BLOCKS of the end-to-end leg (0 = library default)")
     ap.add_argument("--shard", default="replicas", choices=["replicas", "subband"],
                     help="N > 1: one observation per GPU (weak scaling, default) or the subbands of one "
                          "observation split over the GPUs (strong scaling); neither has a collective")
@@ -290,6 +292,8 @@ def main():
         cdmt.cdmt_plan_set_option(plan, cdmt.OPT_DM_TILE, args.dm_tile)
     if args.fused_kernel:
         cdmt.cdmt_plan_set_option(plan, cdmt.OPT_FUSED_KERNEL, args.fused_kernel)
+    if args.host_group_blocks:
+        cdmt.cdmt_plan_set_option(plan, cdmt.OPT_HOST_GROUP_BLOCKS, args.host_group_blocks)
     q = cdmt.cdmt_plan_query(plan, cfg.nsamp)
     nch = cfg.nsub * cfg.nchan
     nt = q["nout_per_chan"]
