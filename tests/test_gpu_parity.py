@@ -310,3 +310,41 @@ def test_fused_kernels_are_bit_reproducible(cdmt, kern):
     for _ in range(20):
         again = cdmt.run_on_device(plan, d_in, cfg.nsamp)
         assert torch.equal(first, again)
+
+
+def test_execute_is_cuda_graph_capturable(cdmt):
+    """cdmt_execute only queues kernels on the caller's stream (no host synchronisation, no allocation,
+    constants uploaded through kernel parameters): it can be captured into a CUDA graph and replayed on
+    new input in the same buffers."""
+    cfg = synth.small_config(nsub=2, nsamp=2 ** 17, nfft=65536, noverlap=16384, nchan=16, ndec=16,
+                             dm=(0.0, 3.0, 11.5))
+    x1 = synth.generate(cfg)
+    cfg2 = synth.small_config(nsub=2, nsamp=2 ** 17, nfft=65536, noverlap=16384, nchan=16, ndec=16,
+                              dm=(0.0, 3.0, 11.5), seed=77)
+    x2 = synth.generate(cfg2)
+    plan = cdmt.cdmt_plan_create(**cfg.plan_kwargs())
+    q = cdmt.cdmt_plan_query(plan, cfg.nsamp)
+    d_in = torch.from_numpy(x1).cuda()
+    nch = cfg.nsub * cfg.nchan
+    out = torch.zeros((cfg.ndm, q["nout_per_chan"], nch), dtype=torch.float32, device="cuda")
+    ws = torch.empty(q["workspace_bytes"], dtype=torch.uint8, device="cuda")
+    eager = cdmt.run_on_device(plan, d_in, cfg.nsamp).clone()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        cdmt.cdmt_execute(plan, d_in, cfg.nsamp, cfg.nsamp, out, out[0].numel(), ws, ws.numel(), side)   # warm up
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        cdmt.cdmt_execute(plan, d_in, cfg.nsamp, cfg.nsamp, out, out[0].numel(), ws, ws.numel(),
+                          torch.cuda.current_stream())
+    out.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(out, eager)
+    d_in.copy_(torch.from_numpy(x2).cuda())
+    g.replay()
+    torch.cuda.synchronize()
+    want = orc.run(orc.Params(**cfg2.plan_kwargs()), x2)
+    check_filterbank(out.cpu().numpy(), want)
