@@ -437,7 +437,8 @@ def main():
                      "frac": adds / ims / 1e9 / peak_add, "bound": "alu",
                      "peak_source": "derived: 148 SM x 128 FP32 lanes x 1.965 GHz (one FADD per lane and clock)",
                      "out_bytes": int(d_ts.numel() * 4),
-                     "note": "cdmt_incoherent_dedisperse on the step's filterbanks; not included in value"}
+                     "note": "cdmt_incoherent_dedisperse on the step's filterbanks; not included in value; `adds` is "
+                             "the count of the brute-force definition (the kernel shares sums between trials)"}
             del d_ts, d_iws
         except Exception as e:
             incoh = {"error": str(e)}
