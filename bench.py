@@ -27,7 +27,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-from paper_1607_00909_b200 import synth  # noqa: E402
+import cdmt_synth as synth  # noqa: E402
 
 METRIC = "input_samples_x_dm_trials_per_s"
 UNIT = "samples*DM/s"

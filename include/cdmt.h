@@ -23,7 +23,9 @@
  *
  * Conventions
  *  - Pointers named d_* are DEVICE pointers, h_* are HOST pointers.  The caller owns all of
- *    them; the library never allocates device memory.  A plan owns only host state.
+ *    them; the library never allocates device memory.  A plan owns host state, plus -- created
+ *    lazily, destroyed with the plan -- the CUDA events of CDMT_OPT_PROFILE and the two copy
+ *    streams and ordering events of the host-buffer path.
  *  - Every entry point returns a CDMT_* status and never aborts or throws.  All arguments
  *    are validated on the host before anything is launched.
  *  - cdmt_execute and the stage calls are asynchronous on `cuda_stream` (a cudaStream_t
@@ -66,8 +68,16 @@ enum {
                                   (chirp of the next trial formed in the shadow of the block barrier); 2 to 5
                                   make cdmt_execute fail with CDMT_ERR_CUDA where they do not apply */
     CDMT_OPT_FORCE_GENERIC = 4, /* older name of the same key (value 1) */
-    CDMT_OPT_HOST_GROUP_BLOCKS = 5 /* cdmt_execute_host: blocks staged per group (0 = about 512 MiB of output) */
+    CDMT_OPT_HOST_GROUP_BLOCKS = 5, /* cdmt_execute_host: blocks staged per group (0 = about 512 MiB of output) */
+    CDMT_OPT_KEEP_TABLES = 6  /* 1: the caller promises that nothing but this plan's executes writes to
+                                 d_workspace between calls that pass the same workspace pointer; the DM list,
+                                 centre frequencies and twiddle tables at its head are then written by the
+                                 first such execute only (default 0: every execute rewrites them with one
+                                 extra small launch).  Setting the option (to either value) forgets the
+                                 remembered workspace. */
 };
+
+enum { CDMT_OUT_F32 = 0, CDMT_OUT_U8 = 1 };           /* host path: float32 filterbanks / redigitised to 8 bit */
 
 /*
  * Create a plan ("user-defined choices" n_c, N_bin, n_d and the DM list).
@@ -110,10 +120,10 @@ int cdmt_plan_query(const cdmt_plan *plan, long long nsamp, int *nblock,
  * Run the whole hot path on device-resident input.
  *   d_in           DEVICE, [nsub][2 pols][..] complex words of the plan's in_dtype, time
  *                  fastest; row (s, p) starts at element (2 s + p) * in_stride_pol.
- *                  16-byte aligned.
+ *                  Aligned to one complex word (8 bytes float32, 2 bytes int8); 16-byte aligned
+ *                  rows let the int8 path use wider loads.
  *   nsamp          samples per row to process (>= nfft)
- *   in_stride_pol  distance between consecutive rows, in complex samples (>= nsamp; even for
- *                  CDMT_IN_CF32 so that every row is 16-byte aligned)
+ *   in_stride_pol  distance between consecutive rows, in complex samples (>= nsamp)
  *   d_out          DEVICE float32, DM plane d starts at d * out_stride_dm elements; inside a
  *                  plane [nblock*Vd][nsub*nchan].  Every element of every plane is written.
  *   out_stride_dm  elements between DM planes (>= nblock*Vd*nsub*nchan)
@@ -128,23 +138,56 @@ int cdmt_execute(cdmt_plan *plan, const void *d_in, long long nsamp, long long i
                  size_t workspace_bytes, void *cuda_stream);
 
 /*
- * The same path with HOST buffers (PAPER.md:93-94, 107: read block, copy to device, ...,
- * copy to host).  h_in / h_out have the layouts of d_in / d_out (h_out planes dense:
- * stride nblock*Vd*nsub*nchan) and should be pinned for full copy speed.  The caller lends
- * device scratch `d_scratch` of at least cdmt_host_scratch_bytes(); input, workspace and
- * output are staged there in groups of blocks, input and output double-buffered
- * (the transfers, not the kernels, are the paper's bottleneck).  Kernels run on
- * `cuda_stream`; the host-to-device copy of the next group and the device-to-host copy of the
- * previous one run meanwhile on two streams the plan creates on first use (ordered after the
- * work already queued on `cuda_stream`).  The call returns after the last device-to-host copy
- * has completed; on error all three streams are drained before it returns.
+ * cdmt_execute that also returns the "block sums" of Alg. 1 l.104:
+ *   d_segsum   DEVICE fp64 [ndm][nblock][nsub*nchan][2] = (sum I, sum I^2) over the Vd float32
+ *              samples that block b gave channel j (output order) at trial d; dense;
+ *              cdmt_redigitize_workspace_bytes() bytes, 16-byte aligned.
+ * The packed fused kernels take the sums from the values they are about to store (each CTA owns
+ * exactly one such segment), so the filterbank is not read back for them; for shapes that run on the
+ * general kernels the sums come from a separate pass over d_out.  Feed them to
+ * cdmt_redigitize_sums.  Same errors as cdmt_execute.
  */
+int cdmt_execute_sums(cdmt_plan *plan, const void *d_in, long long nsamp, long long in_stride_pol,
+                      float *d_out, long long out_stride_dm, double *d_segsum, void *d_workspace,
+                      size_t workspace_bytes, void *cuda_stream);
+
+/*
+ * The same path with HOST buffers (PAPER.md:93-94, 104-108: read block, copy to device, ...,
+ * redigitize, copy to host).  The observation is staged through device scratch in groups of
+ * blocks, input and output double-buffered (the transfers, not the kernels, are the
+ * paper's bottleneck).  Kernels run on `cuda_stream`; the host-to-device copy of the next group
+ * and the device-to-host copy of the previous one run meanwhile on two streams the plan creates on
+ * first use (ordered after the work already queued on `cuda_stream`).
+ *
+ * cdmt_execute_host_async only queues work: it returns at once, and `cuda_stream` is made to wait
+ * for both copy streams at the end, so the results are complete when the work queued on
+ * `cuda_stream` is (synchronise it, or record an event on it).  The host buffers and d_scratch
+ * must stay untouched until then.
+ *   h_in        HOST, layout of d_in (cdmt_execute); pinned memory for full copy speed
+ *   out_kind    CDMT_OUT_F32: h_out is float32 [ndm][nblock*Vd][nsub*nchan] (dense planes), the
+ *               output of cdmt_execute; h_offset / h_scale / qmean / qstd are ignored.
+ *               CDMT_OUT_U8 (Alg. 1 l.104-108): h_out is uint8 with the same shape, redigitised
+ *               group by group -- the batch whose statistics are taken is the
+ *               group of blocks staged together -- with the mapping of cdmt_redigitize;
+ *               h_offset / h_scale are float32 [ngroups][ndm][nsub*nchan].
+ *   d_scratch   DEVICE, 256-byte aligned, >= scratch_bytes of cdmt_host_layout for this out_kind
+ * cdmt_host_layout (host arithmetic; any output pointer may be NULL): device scratch needed, the
+ * number of groups and blocks per group (the last group may be shorter), and the bytes one call
+ * copies host-to-device (each group re-sends the noverlap samples it shares with the previous
+ * one) and device-to-host.
+ * cdmt_execute_host = cdmt_execute_host_async(CDMT_OUT_F32) followed by a wait on all three
+ * streams; cdmt_host_scratch_bytes / cdmt_host_traffic_bytes = cdmt_host_layout(CDMT_OUT_F32).
+ * Errors: CDMT_ERR_ARG, CDMT_ERR_SIZE, CDMT_ERR_WORKSPACE (scratch too small), CDMT_ERR_CUDA.
+ */
+int cdmt_execute_host_async(cdmt_plan *plan, const void *h_in, long long nsamp, long long in_stride_pol,
+                            int out_kind, void *h_out, float *h_offset, float *h_scale, double qmean,
+                            double qstd, void *d_scratch, size_t scratch_bytes, void *cuda_stream);
+int cdmt_host_layout(const cdmt_plan *plan, long long nsamp, int out_kind, size_t *scratch_bytes,
+                     int *ngroups, int *group_blocks, size_t *h2d_bytes, size_t *d2h_bytes);
 int cdmt_execute_host(cdmt_plan *plan, const void *h_in, long long nsamp,
                       long long in_stride_pol, float *h_out, void *d_scratch,
                       size_t scratch_bytes, void *cuda_stream);
 int cdmt_host_scratch_bytes(const cdmt_plan *plan, long long nsamp, size_t *scratch_bytes);
-/* Bytes one cdmt_execute_host call copies host-to-device (each group re-sends the noverlap
- * samples it shares with the previous one) and device-to-host.  Host arithmetic. */
 int cdmt_host_traffic_bytes(const cdmt_plan *plan, long long nsamp, size_t *h2d_bytes, size_t *d2h_bytes);
 
 /*
@@ -189,6 +232,11 @@ int cdmt_redigitize(cdmt_plan *plan, const float *d_fb, long long fb_stride_dm, 
                     float *d_offset, float *d_scale, void *d_workspace, size_t workspace_bytes,
                     void *cuda_stream);
 int cdmt_redigitize_workspace_bytes(const cdmt_plan *plan, long long nblock, size_t *workspace_bytes);
+/* Alg. 1 l.105-106 only, from block sums already taken (cdmt_execute_sums): reads the filterbank once
+ * (4 bytes read, 1 byte written per sample).  d_segsum as in cdmt_execute_sums; two kernels. */
+int cdmt_redigitize_sums(cdmt_plan *plan, const float *d_fb, long long fb_stride_dm, long long nblock,
+                         double qmean, double qstd, const double *d_segsum, unsigned char *d_codes,
+                         long long codes_stride_dm, float *d_offset, float *d_scale, void *cuda_stream);
 
 /*
  * Incoherent dedispersion of the coherently dedispersed filterbanks over a grid of fine DM offsets:
@@ -254,7 +302,9 @@ int cdmt_measure_fp32_peak(void *d_scratch, size_t scratch_bytes, int iters, dou
 /* With CDMT_OPT_PROFILE = 1 every execute records CUDA events on its stream round (kind 0) the
  * two forward-FFT passes of a chunk and (kind 1) each fused per-DM kernel launch.  This call
  * waits for the recorded events, returns the summed durations in milliseconds and the number of
- * spans of each kind since the previous read, and resets the record. */
+ * spans of each kind since the previous read, and resets the record.  Nothing is recorded while
+ * the stream is being captured into a CUDA graph; a record that is never read is discarded once it
+ * holds 8192 spans. */
 int cdmt_profile_read(cdmt_plan *plan, double *ms_forward, double *ms_fused,
                       long long *n_forward, long long *n_fused);
 

@@ -21,12 +21,15 @@ IN_CF32, IN_CI8 = 0, 1
 REF_CHANNEL, REF_SUBBAND = 0, 1
 OPT_CHUNK_UNITS, OPT_DM_TILE, OPT_ACCURATE_SINCOS, OPT_PROFILE, OPT_FORCE_GENERIC = 0, 1, 2, 3, 4
 OPT_HOST_GROUP_BLOCKS = 5
+OPT_KEEP_TABLES = 6
+OUT_F32, OUT_U8 = 0, 1
 OPT_FUSED_KERNEL = 4  # 0 auto, 1 general, 2 scalar fast, 3 packed half transforms + TMEM, 4 packed polarisations + TMEM
 
 EXPORTS = [
     "cdmt_plan_create", "cdmt_plan_destroy", "cdmt_plan_set_option", "cdmt_plan_query",
-    "cdmt_execute", "cdmt_execute_host", "cdmt_host_scratch_bytes", "cdmt_host_traffic_bytes", "cdmt_unpack",
-    "cdmt_forward_spectrum", "cdmt_redigitize", "cdmt_redigitize_workspace_bytes",
+    "cdmt_execute", "cdmt_execute_sums", "cdmt_execute_host", "cdmt_execute_host_async", "cdmt_host_layout",
+    "cdmt_host_scratch_bytes", "cdmt_host_traffic_bytes", "cdmt_unpack",
+    "cdmt_forward_spectrum", "cdmt_redigitize", "cdmt_redigitize_sums", "cdmt_redigitize_workspace_bytes",
     "cdmt_incoherent_query", "cdmt_incoherent_shifts", "cdmt_incoherent_dedisperse",
     "cdmt_sweep_seconds", "cdmt_min_overlap", "cdmt_suggest_sizes",
     "cdmt_measure_fp32_peak", "cdmt_last_launch_count", "cdmt_profile_read", "cdmt_strerror",
@@ -48,7 +51,12 @@ _lib.cdmt_plan_set_option.argtypes = [_vp, _i, _ll]
 _lib.cdmt_plan_query.argtypes = [_vp, _ll, C.POINTER(_i), C.POINTER(_ll), C.POINTER(_ll),
                                  C.POINTER(_sz), C.POINTER(_sz)]
 _lib.cdmt_execute.argtypes = [_vp, _vp, _ll, _ll, _vp, _ll, _vp, _sz, _vp]
+_lib.cdmt_execute_sums.argtypes = [_vp, _vp, _ll, _ll, _vp, _ll, _vp, _vp, _sz, _vp]
 _lib.cdmt_execute_host.argtypes = [_vp, _vp, _ll, _ll, _vp, _vp, _sz, _vp]
+_lib.cdmt_execute_host_async.argtypes = [_vp, _vp, _ll, _ll, _i, _vp, _vp, _vp, _d, _d, _vp, _sz, _vp]
+_lib.cdmt_host_layout.argtypes = [_vp, _ll, _i, C.POINTER(_sz), C.POINTER(_i), C.POINTER(_i), C.POINTER(_sz),
+                                  C.POINTER(_sz)]
+_lib.cdmt_redigitize_sums.argtypes = [_vp, _vp, _ll, _ll, _d, _d, _vp, _vp, _ll, _vp, _vp, _vp]
 _lib.cdmt_host_scratch_bytes.argtypes = [_vp, _ll, C.POINTER(_sz)]
 _lib.cdmt_host_traffic_bytes.argtypes = [_vp, _ll, C.POINTER(_sz), C.POINTER(_sz)]
 _lib.cdmt_unpack.argtypes = [_vp, _vp, _ll, _ll, _vp, _vp]
@@ -169,6 +177,30 @@ def cdmt_execute(plan: Plan, d_in, nsamp: int, in_stride_pol: int, d_out, out_st
     _check(st, "cdmt_execute")
 
 
+def cdmt_execute_sums(plan: Plan, d_in, nsamp: int, in_stride_pol: int, d_out, out_stride_dm: int, d_segsum,
+                      d_workspace, workspace_bytes: int, stream=None):
+    st = _lib.cdmt_execute_sums(plan.handle, _ptr(d_in), int(nsamp), int(in_stride_pol), _ptr(d_out),
+                                int(out_stride_dm), _ptr(d_segsum), _ptr(d_workspace), int(workspace_bytes),
+                                _stream(stream))
+    _check(st, "cdmt_execute_sums")
+
+
+def cdmt_host_layout(plan: Plan, nsamp: int, out_kind: int = OUT_F32) -> dict:
+    sb, ng, gb, a, b = _sz(), _i(), _i(), _sz(), _sz()
+    _check(_lib.cdmt_host_layout(plan.handle, int(nsamp), int(out_kind), C.byref(sb), C.byref(ng), C.byref(gb),
+                                 C.byref(a), C.byref(b)), "cdmt_host_layout")
+    return dict(scratch_bytes=sb.value, ngroups=ng.value, group_blocks=gb.value, h2d_bytes=a.value,
+                d2h_bytes=b.value)
+
+
+def cdmt_execute_host_async(plan: Plan, h_in, nsamp: int, in_stride_pol: int, out_kind: int, h_out, h_offset,
+                            h_scale, qmean: float, qstd: float, d_scratch, scratch_bytes: int, stream=None):
+    st = _lib.cdmt_execute_host_async(plan.handle, _ptr(h_in), int(nsamp), int(in_stride_pol), int(out_kind),
+                                      _ptr(h_out), _ptr(h_offset), _ptr(h_scale), float(qmean), float(qstd),
+                                      _ptr(d_scratch), int(scratch_bytes), _stream(stream))
+    _check(st, "cdmt_execute_host_async")
+
+
 def cdmt_host_scratch_bytes(plan: Plan, nsamp: int) -> int:
     n = _sz()
     _check(_lib.cdmt_host_scratch_bytes(plan.handle, int(nsamp), C.byref(n)), "cdmt_host_scratch_bytes")
@@ -214,6 +246,14 @@ def cdmt_redigitize(plan: Plan, d_fb, fb_stride_dm: int, nblock: int, qmean: flo
                               _ptr(d_codes), int(codes_stride_dm), _ptr(d_offset), _ptr(d_scale),
                               _ptr(d_workspace), int(workspace_bytes), _stream(stream))
     _check(st, "cdmt_redigitize")
+
+
+def cdmt_redigitize_sums(plan: Plan, d_fb, fb_stride_dm: int, nblock: int, qmean: float, qstd: float, d_segsum,
+                         d_codes, codes_stride_dm: int, d_offset, d_scale, stream=None):
+    st = _lib.cdmt_redigitize_sums(plan.handle, _ptr(d_fb), int(fb_stride_dm), int(nblock), float(qmean),
+                                   float(qstd), _ptr(d_segsum), _ptr(d_codes), int(codes_stride_dm),
+                                   _ptr(d_offset), _ptr(d_scale), _stream(stream))
+    _check(st, "cdmt_redigitize_sums")
 
 
 def _ddm(ddm):

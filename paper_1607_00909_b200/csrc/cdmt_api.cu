@@ -20,6 +20,9 @@ struct cdmt_plan {
     int profile;             // record CUDA events around each kernel class
     long long host_group;    // CDMT_OPT_HOST_GROUP_BLOCKS: blocks per staged group of the host path (0 = automatic)
     int force_generic;       // CDMT_OPT_FUSED_KERNEL: 0 auto, 1 generic, 2 scalar fast, 3 packed halves, 4 packed pols, 5 pipelined
+    int keep_tables;         // CDMT_OPT_KEEP_TABLES: the caller leaves the workspace head alone between calls
+    const void *tables_ws;   // workspace whose head holds this plan's tables (keep_tables only)
+    long long tables_cu;     // ... laid out for this many chunk units
     long long last_launches;
     std::vector<cudaEvent_t> ev_pool;   // created lazily, reused
     size_t ev_used;
@@ -29,7 +32,7 @@ struct cdmt_plan {
     IncoherentTables ic;     // incoherent-dedispersion tables of the last fine-DM list used
     std::vector<double> ic_ddm;
     cudaStream_t s_in, s_out;
-    cudaEvent_t ev_start, ev_h2d[2], ev_comp[2], ev_d2h[2];
+    cudaEvent_t ev_start, ev_h2d[2], ev_comp[2], ev_d2h[2], ev_join[2];
     bool host_ready;
 };
 
@@ -43,7 +46,8 @@ static bool plan_host_pipeline(cdmt_plan *p)
     for (int i = 0; i < 2 && ok; ++i)
         ok = cudaEventCreateWithFlags(&p->ev_h2d[i], cudaEventDisableTiming) == cudaSuccess &&
              cudaEventCreateWithFlags(&p->ev_comp[i], cudaEventDisableTiming) == cudaSuccess &&
-             cudaEventCreateWithFlags(&p->ev_d2h[i], cudaEventDisableTiming) == cudaSuccess;
+             cudaEventCreateWithFlags(&p->ev_d2h[i], cudaEventDisableTiming) == cudaSuccess &&
+             cudaEventCreateWithFlags(&p->ev_join[i], cudaEventDisableTiming) == cudaSuccess;
     p->host_ready = ok;
     return ok;
 }
@@ -58,6 +62,8 @@ static cudaEvent_t plan_event(cdmt_plan *p, size_t *idx)
     *idx = p->ev_used;
     return p->ev_pool[p->ev_used++];
 }
+
+constexpr size_t PROFILE_MAX_SPANS = 8192;  // unread profile spans kept per plan
 
 static bool is_pow2(long long x) { return x > 0 && (x & (x - 1)) == 0; }
 
@@ -146,6 +152,9 @@ extern "C" int cdmt_plan_create(cdmt_plan **plan, int nsub, const double *fcen_m
     p->last_launches = 0;
     p->host_ready = false;
     p->host_group = 0;
+    p->keep_tables = 0;
+    p->tables_ws = nullptr;
+    p->tables_cu = 0;
     p->s_in = p->s_out = nullptr;
     *plan = p;
     return CDMT_OK;
@@ -163,6 +172,7 @@ extern "C" int cdmt_plan_destroy(cdmt_plan *plan)
             cudaEventDestroy(plan->ev_h2d[i]);
             cudaEventDestroy(plan->ev_comp[i]);
             cudaEventDestroy(plan->ev_d2h[i]);
+            cudaEventDestroy(plan->ev_join[i]);
         }
     }
     delete plan;
@@ -196,6 +206,11 @@ extern "C" int cdmt_plan_set_option(cdmt_plan *plan, int key, long long value)
     case CDMT_OPT_HOST_GROUP_BLOCKS:
         if (value < 0 || value > (1LL << 30)) return CDMT_ERR_ARG;
         plan->host_group = value;
+        return CDMT_OK;
+    case CDMT_OPT_KEEP_TABLES:
+        if (value != 0 && value != 1) return CDMT_ERR_ARG;
+        plan->keep_tables = (int)value;
+        plan->tables_ws = nullptr;
         return CDMT_OK;
     default: return CDMT_ERR_ARG;
     }
@@ -248,15 +263,17 @@ static int check_cuda(cudaError_t e)
 }
 
 static int validate_input(const cdmt_plan *plan, const void *d_in, long long nsamp, long long in_stride_pol,
-                          long long *nb)
+                          long long *nb, bool align16 = false)
 {
     if (!plan || !d_in) return CDMT_ERR_ARG;
-    if ((reinterpret_cast<uintptr_t>(d_in) & 15) != 0) return CDMT_ERR_ARG;
     const Geometry &g = plan->g;
+    // one complex word: the forward pass reads 8-byte (float32) or 2-byte (int8) words and takes wider
+    // loads only where the address allows; cdmt_unpack's float4 path wants 16 bytes (align16)
+    const uintptr_t word = g.in_dtype == CDMT_IN_CF32 ? (align16 ? 16 : 8) : 2;
+    if ((reinterpret_cast<uintptr_t>(d_in) & (word - 1)) != 0) return CDMT_ERR_ARG;
     if (nsamp < g.nfft) return CDMT_ERR_SIZE;
     if (in_stride_pol < nsamp) return CDMT_ERR_SIZE;
-    // float32 rows are read with 16-byte vector loads: the row stride must be even
-    if (g.in_dtype == CDMT_IN_CF32 && (in_stride_pol & 1)) return CDMT_ERR_SIZE;
+    if (align16 && g.in_dtype == CDMT_IN_CF32 && (in_stride_pol & 1)) return CDMT_ERR_SIZE;
     *nb = nblock_for(g, nsamp);
     if (*nb < 1 || *nb * g.nsub > (1LL << 30)) return CDMT_ERR_SIZE;
     return CDMT_OK;
@@ -264,7 +281,7 @@ static int validate_input(const cdmt_plan *plan, const void *d_in, long long nsa
 
 static int run_chunks(cdmt_plan *plan, const void *d_in, long long in_stride_pol, long long nb, float *d_out,
                       long long out_stride_dm, float2 *d_spec_out, void *d_workspace, size_t workspace_bytes,
-                      cudaStream_t st)
+                      cudaStream_t st, double *d_segsum = nullptr)
 {
     const Geometry &g = plan->g;
     const long long nunits = nb * g.nsub;
@@ -273,13 +290,31 @@ static int run_chunks(cdmt_plan *plan, const void *d_in, long long in_stride_pol
     const size_t need = workspace_layout(g, (int)cu, reinterpret_cast<char *>(d_workspace), &ws);
     if (workspace_bytes < need) return CDMT_ERR_WORKSPACE;
     plan->last_launches = 0;
-    int rc = check_cuda(launch_init_tables(g, ws, plan->dm.data(), plan->fcen.data(), st, &plan->last_launches));
-    if (rc) return rc;
+    int rc = CDMT_OK;
+    if (!(plan->keep_tables && plan->tables_ws == d_workspace && plan->tables_cu == cu)) {
+        rc = check_cuda(launch_init_tables(g, ws, plan->dm.data(), plan->fcen.data(), st, &plan->last_launches));
+        if (rc) return rc;
+        plan->tables_ws = plan->keep_tables ? d_workspace : nullptr;
+        plan->tables_cu = cu;
+    }
+    // no event timing inside a stream capture (the events could not be read back), and an unread
+    // record is overwritten rather than grown without bound
+    bool profile = plan->profile != 0;
+    if (profile) {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) profile = false;
+        cudaGetLastError();
+        if (plan->spans.size() > PROFILE_MAX_SPANS) {
+            plan->spans.clear();
+            plan->ev_used = 0;
+        }
+    }
     auto mark = [&](size_t *idx) -> bool {
-        if (!plan->profile) return true;
+        if (!profile) return true;
         cudaEvent_t e = plan_event(plan, idx);
         return e && cudaEventRecord(e, st) == cudaSuccess;
     };
+    bool sums_done = true;   // cleared by a fused launch that cannot take the block sums itself
     for (long long u0 = 0; u0 < nunits; u0 += cu) {
         const int n = (int)((nunits - u0 < cu) ? nunits - u0 : cu);
         float2 *spec = d_spec_out ? d_spec_out + (size_t)u0 * 2 * g.nfft : ws.spec;
@@ -288,16 +323,19 @@ static int run_chunks(cdmt_plan *plan, const void *d_in, long long in_stride_pol
         rc = check_cuda(launch_forward(g, ws, d_in, in_stride_pol, (int)u0, n, spec, st, &plan->last_launches));
         if (rc) return rc;
         if (!mark(&b)) return check_cuda(cudaErrorUnknown);
-        if (plan->profile) plan->spans.push_back({a, b, 0});
+        if (profile) plan->spans.push_back({a, b, 0});
         if (d_out) {
             rc = check_cuda(launch_fused(g, ws, spec, (int)u0, n, d_out, out_stride_dm, plan->dm_tile,
                                          plan->accurate, plan->force_generic, plan->dm.data(),
-                                         plan->fcen.data(), st, &plan->last_launches));
+                                         plan->fcen.data(), d_segsum, (int)nb, &sums_done, st,
+                                         &plan->last_launches));
             if (rc) return rc;
             if (!mark(&c)) return check_cuda(cudaErrorUnknown);
-            if (plan->profile) plan->spans.push_back({b, c, 1});
+            if (profile) plan->spans.push_back({b, c, 1});
         }
     }
+    if (d_out && d_segsum && !sums_done)
+        return check_cuda(launch_block_sums(g, d_out, out_stride_dm, nb, d_segsum, st, &plan->last_launches));
     return CDMT_OK;
 }
 
@@ -345,6 +383,24 @@ extern "C" int cdmt_execute(cdmt_plan *plan, const void *d_in, long long nsamp, 
                       static_cast<cudaStream_t>(cuda_stream));
 }
 
+extern "C" int cdmt_execute_sums(cdmt_plan *plan, const void *d_in, long long nsamp, long long in_stride_pol,
+                                 float *d_out, long long out_stride_dm, double *d_segsum, void *d_workspace,
+                                 size_t workspace_bytes, void *cuda_stream)
+{
+    long long nb = 0;
+    int rc = validate_input(plan, d_in, nsamp, in_stride_pol, &nb);
+    if (rc) return rc;
+    if (!d_out || !d_workspace || !d_segsum) return CDMT_ERR_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_workspace) & 255) != 0) return CDMT_ERR_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_out) & 3) != 0 || (reinterpret_cast<uintptr_t>(d_segsum) & 15) != 0)
+        return CDMT_ERR_ARG;
+    const Geometry &g = plan->g;
+    if (out_stride_dm < nb * g.vdec * (long long)g.nsub * g.nchan) return CDMT_ERR_SIZE;
+    if (nb > 65535 || g.ndm > 65535) return CDMT_ERR_SIZE;   // grid limits of the stand-alone block-sum pass
+    return run_chunks(plan, d_in, in_stride_pol, nb, d_out, out_stride_dm, nullptr, d_workspace, workspace_bytes,
+                      static_cast<cudaStream_t>(cuda_stream), d_segsum);
+}
+
 extern "C" int cdmt_forward_spectrum(cdmt_plan *plan, const void *d_in, long long nsamp, long long in_stride_pol,
                                      void *d_spec, void *d_workspace, size_t workspace_bytes, void *cuda_stream)
 {
@@ -362,7 +418,7 @@ extern "C" int cdmt_unpack(cdmt_plan *plan, const void *d_in, long long nsamp, l
                            void *d_blocks, void *cuda_stream)
 {
     long long nb = 0;
-    int rc = validate_input(plan, d_in, nsamp, in_stride_pol, &nb);
+    int rc = validate_input(plan, d_in, nsamp, in_stride_pol, &nb, true);
     if (rc) return rc;
     if (!d_blocks || (reinterpret_cast<uintptr_t>(d_blocks) & 15) != 0) return CDMT_ERR_ARG;
     plan->last_launches = 0;
@@ -390,16 +446,20 @@ static long long host_group_blocks(const cdmt_plan *plan, long long nb)
 
 struct HostLayout {
     size_t in_off[2], in_bytes, ws_off, ws_bytes, out_off[2], out_bytes, total;
-    long long gb, in_rowlen;
+    // CDMT_OUT_U8 only: one float32 filterbank buffer, block sums, doubled code and offset/scale buffers
+    size_t sums_off, sums_bytes, codes_off[2], codes_bytes, osc_off[2], osc_bytes;
+    long long gb, in_rowlen, ngroup;
 };
 
-static int host_layout(const cdmt_plan *plan, long long nsamp, HostLayout *L)
+static int host_layout(const cdmt_plan *plan, long long nsamp, int out_kind, HostLayout *L)
 {
     const Geometry &g = plan->g;
     const long long nb = nblock_for(g, nsamp);
     if (nb < 1) return CDMT_ERR_SIZE;
+    if (out_kind != CDMT_OUT_F32 && out_kind != CDMT_OUT_U8) return CDMT_ERR_ARG;
     const long long esz = g.in_dtype == CDMT_IN_CI8 ? 2 : 8;
     L->gb = host_group_blocks(plan, nb);
+    L->ngroup = (nb + L->gb - 1) / L->gb;
     long long rowlen = (L->gb - 1) * g.step + g.nfft;
     rowlen = (rowlen + 7) & ~7LL;  // keep rows 16-byte aligned for both word sizes
     L->in_rowlen = rowlen;
@@ -411,29 +471,36 @@ static int host_layout(const cdmt_plan *plan, long long nsamp, HostLayout *L)
     L->ws_off = L->in_bytes * nbuf;
     const long long cu = chunk_units_for(plan, L->gb * g.nsub);
     L->ws_bytes = al(workspace_layout(g, (int)cu, nullptr, nullptr));
-    L->out_bytes = al((size_t)g.ndm * L->gb * g.vdec * g.nsub * g.nchan * sizeof(float));
+    const size_t samples = (size_t)g.ndm * L->gb * g.vdec * g.nsub * g.nchan;
+    L->out_bytes = al(samples * sizeof(float));
     L->out_off[0] = L->ws_off + L->ws_bytes;
-    L->out_off[1] = nbuf == 2 ? L->out_off[0] + L->out_bytes : L->out_off[0];
-    L->total = L->out_off[0] + L->out_bytes * nbuf;
+    if (out_kind == CDMT_OUT_F32) {
+        L->out_off[1] = nbuf == 2 ? L->out_off[0] + L->out_bytes : L->out_off[0];
+        L->total = L->out_off[0] + L->out_bytes * nbuf;
+        L->sums_off = L->sums_bytes = L->codes_bytes = L->osc_bytes = 0;
+        L->codes_off[0] = L->codes_off[1] = L->osc_off[0] = L->osc_off[1] = 0;
+        return CDMT_OK;
+    }
+    if (L->gb > 65535 || g.ndm > 65535 || L->gb * g.vdec > 65535LL * 16) return CDMT_ERR_SIZE;
+    L->out_off[1] = L->out_off[0];
+    L->sums_off = L->out_off[0] + L->out_bytes;
+    L->sums_bytes = al(redigitize_workspace_bytes(g, L->gb));
+    L->codes_bytes = al(samples);
+    L->codes_off[0] = L->sums_off + L->sums_bytes;
+    L->codes_off[1] = nbuf == 2 ? L->codes_off[0] + L->codes_bytes : L->codes_off[0];
+    L->osc_bytes = al((size_t)2 * g.ndm * g.nsub * g.nchan * sizeof(float));
+    L->osc_off[0] = L->codes_off[0] + L->codes_bytes * nbuf;
+    L->osc_off[1] = nbuf == 2 ? L->osc_off[0] + L->osc_bytes : L->osc_off[0];
+    L->total = L->osc_off[0] + L->osc_bytes * nbuf;
     return CDMT_OK;
 }
 
-extern "C" int cdmt_host_scratch_bytes(const cdmt_plan *plan, long long nsamp, size_t *scratch_bytes)
-{
-    if (!plan || !scratch_bytes) return CDMT_ERR_ARG;
-    HostLayout L;
-    int rc = host_layout(plan, nsamp, &L);
-    if (rc) return rc;
-    *scratch_bytes = L.total;
-    return CDMT_OK;
-}
-
-// Bytes one cdmt_execute_host call moves over the host link (the overlap between groups is re-sent).
-extern "C" int cdmt_host_traffic_bytes(const cdmt_plan *plan, long long nsamp, size_t *h2d_bytes, size_t *d2h_bytes)
+extern "C" int cdmt_host_layout(const cdmt_plan *plan, long long nsamp, int out_kind, size_t *scratch_bytes,
+                                int *ngroups, int *group_blocks, size_t *h2d_bytes, size_t *d2h_bytes)
 {
     if (!plan) return CDMT_ERR_ARG;
     HostLayout L;
-    int rc = host_layout(plan, nsamp, &L);
+    int rc = host_layout(plan, nsamp, out_kind, &L);
     if (rc) return rc;
     const Geometry &g = plan->g;
     const long long nb = nblock_for(g, nsamp);
@@ -443,20 +510,57 @@ extern "C" int cdmt_host_traffic_bytes(const cdmt_plan *plan, long long nsamp, s
         const long long nbg = (nb - b0 < L.gb) ? nb - b0 : L.gb;
         in += (size_t)((nbg - 1) * g.step + g.nfft) * esz * 2 * g.nsub;
     }
+    const size_t samples = (size_t)g.ndm * (size_t)(nb * g.vdec) * (size_t)g.nsub * g.nchan;
+    if (scratch_bytes) *scratch_bytes = L.total;
+    if (ngroups) *ngroups = (int)L.ngroup;
+    if (group_blocks) *group_blocks = (int)L.gb;
     if (h2d_bytes) *h2d_bytes = in;
-    if (d2h_bytes) *d2h_bytes = (size_t)g.ndm * (size_t)(nb * g.vdec) * (size_t)g.nsub * g.nchan * sizeof(float);
+    if (d2h_bytes)
+        *d2h_bytes = out_kind == CDMT_OUT_F32
+                         ? samples * sizeof(float)
+                         : samples + (size_t)L.ngroup * 2 * g.ndm * g.nsub * g.nchan * sizeof(float);
     return CDMT_OK;
 }
 
-extern "C" int cdmt_execute_host(cdmt_plan *plan, const void *h_in, long long nsamp, long long in_stride_pol,
-                                 float *h_out, void *d_scratch, size_t scratch_bytes, void *cuda_stream)
+extern "C" int cdmt_host_scratch_bytes(const cdmt_plan *plan, long long nsamp, size_t *scratch_bytes)
+{
+    if (!scratch_bytes) return CDMT_ERR_ARG;
+    return cdmt_host_layout(plan, nsamp, CDMT_OUT_F32, scratch_bytes, nullptr, nullptr, nullptr, nullptr);
+}
+
+extern "C" int cdmt_host_traffic_bytes(const cdmt_plan *plan, long long nsamp, size_t *h2d_bytes, size_t *d2h_bytes)
+{
+    return cdmt_host_layout(plan, nsamp, CDMT_OUT_F32, nullptr, nullptr, nullptr, h2d_bytes, d2h_bytes);
+}
+
+// `height` rows of `width` bytes between pitched buffers.  cudaMemcpy2DAsync rejects pitches above
+// cudaDeviceProp::memPitch (2^31 - 1 bytes), which a long observation exceeds: then one copy per row.
+static cudaError_t copy_rows_async(void *dst, size_t dpitch, const void *src, size_t spitch, size_t width,
+                                   size_t height, cudaMemcpyKind kind, cudaStream_t st)
+{
+    const size_t lim = 0x7fffffffu;
+    if (dpitch <= lim && spitch <= lim) return cudaMemcpy2DAsync(dst, dpitch, src, spitch, width, height, kind, st);
+    for (size_t r = 0; r < height; ++r) {
+        cudaError_t e = cudaMemcpyAsync(static_cast<char *>(dst) + r * dpitch, static_cast<const char *>(src) + r * spitch,
+                                        width, kind, st);
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
+extern "C" int cdmt_execute_host_async(cdmt_plan *plan, const void *h_in, long long nsamp, long long in_stride_pol,
+                                       int out_kind, void *h_out, float *h_offset, float *h_scale, double qmean,
+                                       double qstd, void *d_scratch, size_t scratch_bytes, void *cuda_stream)
 {
     if (!plan || !h_in || !h_out || !d_scratch) return CDMT_ERR_ARG;
     if ((reinterpret_cast<uintptr_t>(d_scratch) & 255) != 0) return CDMT_ERR_ARG;
+    const bool u8 = out_kind == CDMT_OUT_U8;
+    if (u8 && (!h_offset || !h_scale || !(qstd > 0.0) || !std::isfinite(qstd) || !std::isfinite(qmean)))
+        return CDMT_ERR_ARG;
     const Geometry &g = plan->g;
     if (nsamp < g.nfft || in_stride_pol < nsamp) return CDMT_ERR_SIZE;
     HostLayout L;
-    int rc = host_layout(plan, nsamp, &L);
+    int rc = host_layout(plan, nsamp, out_kind, &L);
     if (rc) return rc;
     if (scratch_bytes < L.total) return CDMT_ERR_WORKSPACE;
     if (!plan_host_pipeline(plan)) return check_cuda(cudaErrorUnknown);
@@ -466,8 +570,14 @@ extern "C" int cdmt_execute_host(cdmt_plan *plan, const void *h_in, long long ns
     char *base = reinterpret_cast<char *>(d_scratch);
     const size_t nchtot = (size_t)g.nsub * g.nchan;
     const size_t plane_host = (size_t)nb * g.vdec * nchtot;
-    const long long ngroup = (nb + L.gb - 1) / L.gb;
+    const size_t osz = u8 ? 1 : sizeof(float);
+    const long long ngroup = L.ngroup;
     long long launches = 0;
+    // the scratch workspace is ours for the whole call: its tables are written by the first group only
+    const int keep_saved = plan->keep_tables;
+    const void *ws_saved = plan->tables_ws;
+    plan->keep_tables = 1;
+    plan->tables_ws = nullptr;
 
     // the copy streams start after whatever the caller queued on `st` before this call
     rc = check_cuda(cudaEventRecord(plan->ev_start, st));
@@ -484,10 +594,10 @@ extern "C" int cdmt_execute_host(cdmt_plan *plan, const void *h_in, long long ns
             int r = check_cuda(cudaStreamWaitEvent(plan->s_in, plan->ev_comp[k], 0));
             if (r) return r;
         }
-        int r = check_cuda(cudaMemcpy2DAsync(base + L.in_off[k], (size_t)L.in_rowlen * esz,
-                                             reinterpret_cast<const char *>(h_in) + (size_t)b0 * g.step * esz,
-                                             (size_t)in_stride_pol * esz, (size_t)len * esz, (size_t)2 * g.nsub,
-                                             cudaMemcpyHostToDevice, plan->s_in));
+        int r = check_cuda(copy_rows_async(base + L.in_off[k], (size_t)L.in_rowlen * esz,
+                                           reinterpret_cast<const char *>(h_in) + (size_t)b0 * g.step * esz,
+                                           (size_t)in_stride_pol * esz, (size_t)len * esz, (size_t)2 * g.nsub,
+                                           cudaMemcpyHostToDevice, plan->s_in));
         if (r) return r;
         return check_cuda(cudaEventRecord(plan->ev_h2d[k], plan->s_in));
     };
@@ -499,14 +609,23 @@ extern "C" int cdmt_execute_host(cdmt_plan *plan, const void *h_in, long long ns
         const long long nbg = (nb - b0 < L.gb) ? nb - b0 : L.gb;
         const size_t plane_dev = (size_t)nbg * g.vdec * nchtot;
         float *d_out = reinterpret_cast<float *>(base + L.out_off[k]);
-        // compute of group i: needs its input, and output buffer k drained by the copy of group i-2
+        // compute of group i: needs its input, and the buffer the copy of group i-2 read from
         rc = check_cuda(cudaStreamWaitEvent(st, plan->ev_h2d[k], 0));
         if (!rc && i >= 2) rc = check_cuda(cudaStreamWaitEvent(st, plan->ev_d2h[k], 0));
         if (rc) break;
+        double *d_sums = u8 ? reinterpret_cast<double *>(base + L.sums_off) : nullptr;
         rc = run_chunks(plan, base + L.in_off[k], L.in_rowlen, nbg, d_out, (long long)plane_dev, nullptr,
-                        base + L.ws_off, L.ws_bytes, st);
+                        base + L.ws_off, L.ws_bytes, st, d_sums);
         if (rc) break;
         launches += plan->last_launches;
+        unsigned char *d_codes = reinterpret_cast<unsigned char *>(base + L.codes_off[k]);
+        float *d_off = reinterpret_cast<float *>(base + L.osc_off[k]), *d_sc = d_off + (size_t)g.ndm * nchtot;
+        if (u8) {
+            // Alg. 1 l.105-106 on the batch just computed (its block sums came with the filterbank)
+            rc = check_cuda(launch_stats_quantize(g, d_out, (long long)plane_dev, nbg, qmean, qstd, d_sums, d_codes,
+                                                  (long long)plane_dev, d_off, d_sc, st, &launches));
+            if (rc) break;
+        }
         rc = check_cuda(cudaEventRecord(plan->ev_comp[k], st));
         if (rc) break;
         // the next group's input travels while this group computes
@@ -516,16 +635,42 @@ extern "C" int cdmt_execute_host(cdmt_plan *plan, const void *h_in, long long ns
         }
         rc = check_cuda(cudaStreamWaitEvent(plan->s_out, plan->ev_comp[k], 0));
         if (!rc)
-            rc = check_cuda(cudaMemcpy2DAsync(h_out + (size_t)b0 * g.vdec * nchtot, plane_host * sizeof(float), d_out,
-                                              plane_dev * sizeof(float), plane_dev * sizeof(float), (size_t)g.ndm,
-                                              cudaMemcpyDeviceToHost, plan->s_out));
+            rc = check_cuda(copy_rows_async(static_cast<char *>(h_out) + (size_t)b0 * g.vdec * nchtot * osz, plane_host * osz,
+                                            u8 ? static_cast<const void *>(d_codes) : static_cast<const void *>(d_out),
+                                            plane_dev * osz, plane_dev * osz, (size_t)g.ndm, cudaMemcpyDeviceToHost,
+                                            plan->s_out));
+        if (!rc && u8) {
+            const size_t n = (size_t)g.ndm * nchtot;
+            rc = check_cuda(cudaMemcpyAsync(h_offset + (size_t)i * n, d_off, n * sizeof(float), cudaMemcpyDeviceToHost,
+                                            plan->s_out));
+            if (!rc)
+                rc = check_cuda(cudaMemcpyAsync(h_scale + (size_t)i * n, d_sc, n * sizeof(float), cudaMemcpyDeviceToHost,
+                                                plan->s_out));
+        }
         if (!rc) rc = check_cuda(cudaEventRecord(plan->ev_d2h[k], plan->s_out));
     }
     plan->last_launches = launches;
-    // drain all three streams whatever happened, so that the scratch can be reused or freed
-    const int r1 = check_cuda(cudaStreamSynchronize(plan->s_in));
-    const int r2 = check_cuda(cudaStreamSynchronize(st));
-    const int r3 = check_cuda(cudaStreamSynchronize(plan->s_out));
+    plan->keep_tables = keep_saved;
+    plan->tables_ws = ws_saved;
+    // join: whatever was queued on the copy streams completes before later work on `st` (also on error,
+    // so that draining `st` is enough before the buffers are reused or freed)
+    int rj = check_cuda(cudaEventRecord(plan->ev_join[0], plan->s_in));
+    if (!rj) rj = check_cuda(cudaStreamWaitEvent(st, plan->ev_join[0], 0));
+    if (!rj) rj = check_cuda(cudaEventRecord(plan->ev_join[1], plan->s_out));
+    if (!rj) rj = check_cuda(cudaStreamWaitEvent(st, plan->ev_join[1], 0));
+    return rc ? rc : rj;
+}
+
+extern "C" int cdmt_execute_host(cdmt_plan *plan, const void *h_in, long long nsamp, long long in_stride_pol,
+                                 float *h_out, void *d_scratch, size_t scratch_bytes, void *cuda_stream)
+{
+    const int rc = cdmt_execute_host_async(plan, h_in, nsamp, in_stride_pol, CDMT_OUT_F32, h_out, nullptr, nullptr, 0.0,
+                                           1.0, d_scratch, scratch_bytes, cuda_stream);
+    if (rc == CDMT_ERR_ARG || rc == CDMT_ERR_SIZE || rc == CDMT_ERR_WORKSPACE) return rc;   // nothing was queued
+    // drain whatever happened, so that the scratch can be reused or freed
+    const int r1 = plan->host_ready ? check_cuda(cudaStreamSynchronize(plan->s_in)) : CDMT_OK;
+    const int r2 = check_cuda(cudaStreamSynchronize(static_cast<cudaStream_t>(cuda_stream)));
+    const int r3 = plan->host_ready ? check_cuda(cudaStreamSynchronize(plan->s_out)) : CDMT_OK;
     if (rc) return rc;
     return r1 ? r1 : (r2 ? r2 : r3);
 }
@@ -559,6 +704,26 @@ extern "C" int cdmt_redigitize(cdmt_plan *plan, const float *d_fb, long long fb_
     return check_cuda(launch_redigitize(g, d_fb, fb_stride_dm, nblock, qmean, qstd, d_codes, codes_stride_dm, d_offset,
                                         d_scale, d_workspace, static_cast<cudaStream_t>(cuda_stream),
                                         &plan->last_launches));
+}
+
+extern "C" int cdmt_redigitize_sums(cdmt_plan *plan, const float *d_fb, long long fb_stride_dm, long long nblock,
+                                    double qmean, double qstd, const double *d_segsum, unsigned char *d_codes,
+                                    long long codes_stride_dm, float *d_offset, float *d_scale, void *cuda_stream)
+{
+    if (!plan || !d_fb || !d_codes || !d_offset || !d_scale || !d_segsum) return CDMT_ERR_ARG;
+    if (!(qstd > 0.0) || !std::isfinite(qstd) || !std::isfinite(qmean)) return CDMT_ERR_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_fb) & 3) != 0 || (reinterpret_cast<uintptr_t>(d_offset) & 3) != 0 ||
+        (reinterpret_cast<uintptr_t>(d_scale) & 3) != 0 || (reinterpret_cast<uintptr_t>(d_segsum) & 15) != 0)
+        return CDMT_ERR_ARG;
+    const Geometry &g = plan->g;
+    if (nblock < 1 || nblock > 65535 || g.ndm > 65535) return CDMT_ERR_SIZE;
+    const long long plane = nblock * g.vdec * (long long)g.nsub * g.nchan;
+    if (fb_stride_dm < plane || codes_stride_dm < plane) return CDMT_ERR_SIZE;
+    if (nblock * g.vdec > 65535LL * 16) return CDMT_ERR_SIZE;
+    plan->last_launches = 0;
+    return check_cuda(launch_stats_quantize(g, d_fb, fb_stride_dm, nblock, qmean, qstd, d_segsum, d_codes,
+                                            codes_stride_dm, d_offset, d_scale, static_cast<cudaStream_t>(cuda_stream),
+                                            &plan->last_launches));
 }
 
 // ---- incoherent dedispersion over fine DM offsets ----------------------------

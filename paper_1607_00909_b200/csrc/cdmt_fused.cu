@@ -403,8 +403,10 @@ static double phase_cycles_bound(const Geometry &g, const double *h_dm, const do
 
 cudaError_t launch_fused(const Geometry &g, const Workspace &ws, const float2 *spec, int unit0, int nunits,
                          float *d_out, long long out_stride_dm, int dm_tile, int accurate, int force_generic,
-                         const double *h_dm, const double *h_fcen, cudaStream_t st, long long *launches)
+                         const double *h_dm, const double *h_fcen, double *d_segsum, int nblock_total,
+                         bool *sums_done, cudaStream_t st, long long *launches)
 {
+    if (d_segsum && sums_done) *sums_done = false;   // set again by a kernel that takes the sums itself
     const int M = g.mbin, D = g.ndec;
     if (dm_tile <= 0 || dm_tile > g.ndm) dm_tile = g.ndm;
     dim3 grid((unsigned)(nunits * g.nchan), (unsigned)((g.ndm + dm_tile - 1) / dm_tile));
@@ -419,23 +421,21 @@ cudaError_t launch_fused(const Geometry &g, const Workspace &ws, const float2 *s
     int logd = 0;
     while ((1 << logd) < D) ++logd;
     // force_generic carries CDMT_OPT_FUSED_KERNEL: 0 auto, 1 generic, 2 scalar fast, 3 packed halves (x2),
-    // 4 packed pols (pp), 5 packed pols, software-pipelined chirp (sp)
+    // 5 packed pols, software-pipelined chirp (sp)
     const bool fast_ok = !accurate && M >= 512 && D <= 32 && (1 << logd) == D && (g.hdisc % D) == 0 &&
                          poly_phase_ok(g, h_dm, h_fcen);
     // x2 and sp reduce the phase mod 1 with a 2^20 magic number: |phase| must stay below 2^19 cycles
     const bool small_phase = phase_cycles_bound(g, h_dm, h_fcen) < 262144.0;
     const bool x2_ok = fast_ok && small_phase && fused_x2_supported(M, D, g.hdisc);
-    const bool pp_ok = fast_ok && fused_pp_supported(M, D, g.hdisc);
     const bool sp_ok = fast_ok && small_phase && fused_sp_supported(M, D, g.hdisc);
     if (force_generic == 5 && !sp_ok) return cudaErrorInvalidValue;
-    if (force_generic == 4 && !pp_ok) return cudaErrorInvalidValue;
+    if (force_generic == 4) return cudaErrorInvalidValue;
     if (force_generic == 3 && !x2_ok) return cudaErrorInvalidValue;
     if (force_generic == 2 && !fast_ok) return cudaErrorInvalidValue;
     // automatic choice: x2 (measured fastest on all five configs: c3 21.8 ms per launch against 22.2 for sp),
-    // then sp (covers ndec < 8), then pp
+    // then sp (covers ndec < 8)
     if (x2_ok && (force_generic == 0 || force_generic == 3)) return launch_fused_x2(M, logd, fa, h_dm, nunits, st, launches);
     if (sp_ok && (force_generic == 0 || force_generic == 5)) return launch_fused_sp(M, logd, fa, h_dm, nunits, st, launches);
-    if (pp_ok && (force_generic == 0 || force_generic == 4)) return launch_fused_pp(M, logd, fa, h_dm, nunits, st, launches);
     const bool fast = fast_ok && force_generic != 1;
     cudaError_t e = cudaErrorInvalidValue;
     if (fast) {

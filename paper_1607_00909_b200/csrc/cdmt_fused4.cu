@@ -1,14 +1,14 @@
 // cdmt_fused4.cu -- k_fused_sp: the fused per-DM kernel (Alg. 1 l.99-103 + time integration,
 // PAPER.md:117-123), software-pipelined over the DM trials.
 //
-// Same data layout and arithmetic as k_fused_sp (cdmt_fused3.cu): one CTA per (subband, block,
-// channel), both polarisations in the two lanes of packed-FP32 registers, M = 16 * 16 * R2,
-// 16 packed points per thread, spectrum bins and last-pass twiddles in tensor memory.  What
-// changes is WHEN the chirp of Eq. 1 is formed.  In k_fused_sp every trial starts with the
-// FP64 phase polynomial and the MUFU sin/cos of its 16 bins, and all warps of a CTA do so at
-// the same time (they leave the same block barrier), so the FP64/XU pipes and the FP32 pipe
-// take turns instead of overlapping (ncu: FMA pipe 65 % busy, removing the chirp arithmetic
-// or the barrier gives 17 % / 11 %).  Here the block barrier between pass 1 and pass 2 is split
+// One CTA per (subband, block, channel), both polarisations in the two lanes of packed-FP32
+// registers, M = 16 * 16 * R2, 16 packed points per thread, spectrum bins and last-pass twiddles
+// in tensor memory.  The point of the kernel is WHEN the chirp of Eq. 1 is formed.  If every
+// trial starts with the FP64 phase polynomial and the MUFU sin/cos of its 16 bins, all warps of
+// a CTA do so at the same time (they leave the same block barrier), so the FP64/XU pipes and the
+// FP32 pipe take turns instead of overlapping (round-1 ncu of that form: FMA pipe 65 % busy,
+// removing the chirp arithmetic or the barrier gave 17 % / 11 %).  Here the block barrier
+// between pass 1 and pass 2 is split
 // into arrive / wait, and the chirp of trial d+1 is computed between the two -- in the
 // barrier's shadow, while the data registers are dead -- and parked in tensor memory:
 //

@@ -110,11 +110,6 @@ __device__ __forceinline__ void lane_reduce_scatter(float *a, int lane)
 bool fused_x2_supported(int M, int ndec, int hdisc);
 cudaError_t launch_fused_x2(int M, int logd, const FusedArgs &fa, const double *h_dm, int nunits, cudaStream_t st,
                             long long *launches);
-// cdmt_fused3.cu
-bool fused_pp_supported(int M, int ndec, int hdisc);
-cudaError_t launch_fused_pp(int M, int logd, const FusedArgs &fa, const double *h_dm, int nunits, cudaStream_t st,
-                            long long *launches);
-
 // cdmt_fused4.cu
 bool fused_sp_supported(int M, int ndec, int hdisc);
 cudaError_t launch_fused_sp(int M, int logd, const FusedArgs &fa, const double *h_dm, int nunits, cudaStream_t st,

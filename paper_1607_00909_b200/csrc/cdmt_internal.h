@@ -40,9 +40,12 @@ cudaError_t launch_init_tables(const Geometry &g, const Workspace &ws, const dou
 cudaError_t launch_forward(const Geometry &g, const Workspace &ws, const void *d_in,
                            long long in_stride_pol, int unit0, int nunits, float2 *spec_out,
                            cudaStream_t st, long long *launches);
+// d_segsum (may be null): block sums [ndm][nblock_total][nch] x (sum I, sum I^2); *sums_done is cleared if the
+// kernel chosen cannot take them (the caller then runs launch_block_sums over the finished filterbank)
 cudaError_t launch_fused(const Geometry &g, const Workspace &ws, const float2 *spec, int unit0,
                          int nunits, float *d_out, long long out_stride_dm, int dm_tile,
                          int accurate, int force_generic, const double *h_dm, const double *h_fcen,
+                         double *d_segsum, int nblock_total, bool *sums_done,
                          cudaStream_t st, long long *launches);
 cudaError_t launch_unpack(const Geometry &g, const void *d_in, long long in_stride_pol,
                           int nblock, float2 *d_blocks, cudaStream_t st, long long *launches);
@@ -54,6 +57,13 @@ cudaError_t launch_redigitize(const Geometry &g, const float *d_fb, long long fb
                               double qmean, double qstd, unsigned char *d_codes, long long codes_stride_dm,
                               float *d_offset, float *d_scale, void *d_workspace, cudaStream_t st,
                               long long *launches);
+
+cudaError_t launch_block_sums(const Geometry &g, const float *d_fb, long long fb_stride_dm, long long nblock,
+                              double *d_segsum, cudaStream_t st, long long *launches);
+cudaError_t launch_stats_quantize(const Geometry &g, const float *d_fb, long long fb_stride_dm, long long nblock,
+                                  double qmean, double qstd, const double *d_segsum, unsigned char *d_codes,
+                                  long long codes_stride_dm, float *d_offset, float *d_scale, cudaStream_t st,
+                                  long long *launches);
 
 // cdmt_incoherent.cu: incoherent dedispersion of the filterbanks over fine DM offsets
 struct IncoherentTables {            // host side, owned by the plan (must outlive the async upload)

@@ -1,6 +1,6 @@
 // cdmt_kernels.cu -- the sm_100a kernels of the cdmt hot path and their launchers.
 //
-//  k_init_twiddles / k_upload   constant tables into the workspace head
+//  k_init_tables                DM list, centre frequencies and twiddle tables into the workspace head
 //  k_unpack                     Alg. 1 l.95 as a stand-alone stage
 //  k_fwd_pass<L, MODE, IN>      forward FFT of length nfft = n1*n2 as two passes of a four-step
 //                               decomposition; pass A reads the raw voltages (unpack fused into
@@ -15,18 +15,13 @@ namespace cdmt {
 // ------------------------------------------------------------------------------------
 // constant tables
 // ------------------------------------------------------------------------------------
+constexpr int INIT_CHUNK = 1024;  // doubles carried per table in one kernel parameter block
 struct DoubleChunk {
-    double v[256];
+    double v[INIT_CHUNK];
 };
 
-__global__ void k_upload(double *dst, DoubleChunk c, int n)
-{
-    int i = threadIdx.x;
-    if (i < n) dst[i] = c.v[i];
-}
-
-// pass twiddles of RadixPlan<L> (runtime evaluation of the same layout)
-__global__ void k_init_pass_twiddles(float2 *tw, int L, int sign)
+// pass twiddles of RadixPlan<L> (runtime evaluation of the same layout); `nthreads` threads, this one is `t`
+__device__ void init_pass_twiddles(float2 *tw, int L, int sign, int t, int nthreads)
 {
     int log2L = 31 - __clz(L);
     int n16 = log2L / 4, rest = 1 << (log2L % 4);
@@ -36,7 +31,7 @@ __global__ void k_init_pass_twiddles(float2 *tw, int L, int sign)
         int R = p < n16 ? 16 : rest;
         if (p >= 1) {
             int cnt = (R - 1) * ns;
-            for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < cnt; e += gridDim.x * blockDim.x) {
+            for (int e = t; e < cnt; e += nthreads) {
                 int r = e / ns + 1, k = e % ns;
                 double s, c;
                 sincospi(2.0 * (double)k * (double)r / ((double)ns * (double)R), &s, &c);
@@ -49,10 +44,10 @@ __global__ void k_init_pass_twiddles(float2 *tw, int L, int sign)
 }
 
 // four-step twiddles: exp(-2 pi i e / N) = hi[e >> lo_bits] * lo[e & (2^lo_bits - 1)]
-__global__ void k_init_fourstep(float2 *lo, float2 *hi, int N, int lo_bits)
+__device__ void init_fourstep(float2 *lo, float2 *hi, int N, int lo_bits, int t, int nthreads)
 {
     int nlo = 1 << lo_bits, nhi = N >> lo_bits;
-    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < nlo + nhi; e += gridDim.x * blockDim.x) {
+    for (int e = t; e < nlo + nhi; e += nthreads) {
         double s, c;
         if (e < nlo) {
             sincospi(-2.0 * (double)e / (double)N, &s, &c);
@@ -63,6 +58,38 @@ __global__ void k_init_fourstep(float2 *lo, float2 *hi, int N, int lo_bits)
             hi[a] = make_float2((float)c, (float)s);
         }
     }
+}
+
+struct InitArgs {
+    double *dm, *fcen;
+    float2 *tw_n1, *tw_n2, *tw_m, *tw4_lo, *tw4_hi;
+    int n1, n2, mbin, nfft, lo_bits;
+    int dm0, ndm, f0, nf;   // this launch carries dm[dm0, dm0 + ndm) and fcen[f0, f0 + nf)
+    int tables;             // 1: also fill the twiddle tables
+};
+
+// One launch fills the whole head of the workspace: block 0 the DM list, block 1 the centre
+// frequencies (both travel in the kernel parameter block, so that the call stays capturable into
+// a CUDA graph), blocks 2.. the twiddle tables by role (blockIdx % 4).
+__global__ void __launch_bounds__(256)
+k_init_tables(const InitArgs a, const __grid_constant__ DoubleChunk dm, const __grid_constant__ DoubleChunk fc)
+{
+    const int t = threadIdx.x;
+    if (blockIdx.x == 0) {
+        for (int i = t; i < a.ndm; i += 256) a.dm[a.dm0 + i] = dm.v[i];
+        return;
+    }
+    if (blockIdx.x == 1) {
+        for (int i = t; i < a.nf; i += 256) a.fcen[a.f0 + i] = fc.v[i];
+        return;
+    }
+    if (!a.tables) return;
+    const int role = (blockIdx.x - 2) & 3, nb = (gridDim.x - 2) >> 2;
+    const int tt = ((blockIdx.x - 2) >> 2) * 256 + t, nthreads = nb * 256;
+    if (role == 0) init_pass_twiddles(a.tw_n1, a.n1, -1, tt, nthreads);
+    else if (role == 1) init_pass_twiddles(a.tw_n2, a.n2, -1, tt, nthreads);
+    else if (role == 2) init_pass_twiddles(a.tw_m, a.mbin, +1, tt, nthreads);
+    else init_fourstep(a.tw4_lo, a.tw4_hi, a.nfft, a.lo_bits, tt, nthreads);
 }
 
 // ------------------------------------------------------------------------------------
@@ -253,23 +280,23 @@ size_t workspace_layout(const Geometry &g, int chunk_units, char *base, Workspac
 cudaError_t launch_init_tables(const Geometry &g, const Workspace &ws, const double *h_dm,
                                const double *h_fcen, cudaStream_t st, long long *launches)
 {
-    auto upload = [&](double *dst, const double *src, int n) {
-        for (int o = 0; o < n; o += 256) {
-            DoubleChunk c;
-            int cnt = n - o < 256 ? n - o : 256;
-            for (int i = 0; i < cnt; ++i) c.v[i] = src[o + i];
-            for (int i = cnt; i < 256; ++i) c.v[i] = 0.0;
-            k_upload<<<1, 256, 0, st>>>(dst + o, c, cnt);
-            ++*launches;
+    InitArgs a;
+    a.dm = ws.dm; a.fcen = ws.fcen; a.tw_n1 = ws.tw_n1; a.tw_n2 = ws.tw_n2; a.tw_m = ws.tw_m;
+    a.tw4_lo = ws.tw4_lo; a.tw4_hi = ws.tw4_hi;
+    a.n1 = g.n1; a.n2 = g.n2; a.mbin = g.mbin; a.nfft = g.nfft; a.lo_bits = g.lo_bits;
+    // one launch unless a list is longer than a parameter block carries
+    for (int o = 0; o < g.ndm || o < g.nsub || o == 0; o += INIT_CHUNK) {
+        DoubleChunk dm, fc;
+        a.dm0 = o; a.ndm = g.ndm - o < 0 ? 0 : (g.ndm - o < INIT_CHUNK ? g.ndm - o : INIT_CHUNK);
+        a.f0 = o;  a.nf = g.nsub - o < 0 ? 0 : (g.nsub - o < INIT_CHUNK ? g.nsub - o : INIT_CHUNK);
+        for (int i = 0; i < INIT_CHUNK; ++i) {
+            dm.v[i] = i < a.ndm ? h_dm[o + i] : 0.0;
+            fc.v[i] = i < a.nf ? h_fcen[o + i] : 0.0;
         }
-    };
-    upload(ws.dm, h_dm, g.ndm);
-    upload(ws.fcen, h_fcen, g.nsub);
-    k_init_pass_twiddles<<<8, 256, 0, st>>>(ws.tw_n1, g.n1, -1);
-    k_init_pass_twiddles<<<8, 256, 0, st>>>(ws.tw_n2, g.n2, -1);
-    k_init_pass_twiddles<<<32, 256, 0, st>>>(ws.tw_m, g.mbin, +1);
-    k_init_fourstep<<<8, 256, 0, st>>>(ws.tw4_lo, ws.tw4_hi, g.nfft, g.lo_bits);
-    *launches += 4;
+        a.tables = o == 0;
+        k_init_tables<<<a.tables ? 2 + 4 * 8 : 2, 256, 0, st>>>(a, dm, fc);
+        ++*launches;
+    }
     return cudaGetLastError();
 }
 

@@ -147,28 +147,43 @@ size_t redigitize_workspace_bytes(const Geometry &g, long long nblock)
     return sizeof(double2) * (size_t)g.ndm * (size_t)nblock * (size_t)g.nsub * g.nchan;
 }
 
-cudaError_t launch_redigitize(const Geometry &g, const float *d_fb, long long fb_stride_dm, long long nblock,
-                              double qmean, double qstd, unsigned char *d_codes, long long codes_stride_dm,
-                              float *d_offset, float *d_scale, void *d_workspace, cudaStream_t st, long long *launches)
+// float4 / 32-bit paths need 16-byte (4-byte) aligned rows
+static bool fb_vec4(int nch, const float *d_fb, long long fb_stride_dm)
+{
+    return nch % 4 == 0 && fb_stride_dm % 4 == 0 && (reinterpret_cast<uintptr_t>(d_fb) & 15) == 0;
+}
+
+// l.104 as a stand-alone pass over the filterbank (the packed fused kernels take the sums themselves)
+cudaError_t launch_block_sums(const Geometry &g, const float *d_fb, long long fb_stride_dm, long long nblock,
+                              double *d_segsum, cudaStream_t st, long long *launches)
+{
+    const int nch = g.nsub * g.nchan, vd = g.vdec;
+    double2 *segsum = reinterpret_cast<double2 *>(d_segsum);
+    const bool vec4 = fb_vec4(nch, d_fb, fb_stride_dm);
+    const int ngroups = vec4 ? nch / 4 : nch;
+    dim3 grid((unsigned)((ngroups + BS_TX - 1) / BS_TX), (unsigned)nblock, (unsigned)g.ndm), block(BS_TX, BS_TY);
+    if (vec4)
+        k_block_sums<4><<<grid, block, 0, st>>>(d_fb, fb_stride_dm, vd, nch, segsum);
+    else
+        k_block_sums<1><<<grid, block, 0, st>>>(d_fb, fb_stride_dm, vd, nch, segsum);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) ++*launches;
+    return e;
+}
+
+// l.105-106 from given block sums
+cudaError_t launch_stats_quantize(const Geometry &g, const float *d_fb, long long fb_stride_dm, long long nblock,
+                                  double qmean, double qstd, const double *d_segsum, unsigned char *d_codes,
+                                  long long codes_stride_dm, float *d_offset, float *d_scale, cudaStream_t st,
+                                  long long *launches)
 {
     const int nch = g.nsub * g.nchan, vd = g.vdec;
     const long long nt = nblock * vd;
-    double2 *segsum = reinterpret_cast<double2 *>(d_workspace);
-    // float4 / 32-bit paths need 16-byte (4-byte) aligned rows in both arrays
-    const bool vec4 = nch % 4 == 0 && fb_stride_dm % 4 == 0 && codes_stride_dm % 4 == 0 &&
-                      (reinterpret_cast<uintptr_t>(d_fb) & 15) == 0 && (reinterpret_cast<uintptr_t>(d_codes) & 3) == 0 &&
+    const double2 *segsum = reinterpret_cast<const double2 *>(d_segsum);
+    const bool vec4 = fb_vec4(nch, d_fb, fb_stride_dm) && codes_stride_dm % 4 == 0 &&
+                      (reinterpret_cast<uintptr_t>(d_codes) & 3) == 0 &&
                       (reinterpret_cast<uintptr_t>(d_offset) & 15) == 0 && (reinterpret_cast<uintptr_t>(d_scale) & 15) == 0;
     const int ngroups = vec4 ? nch / 4 : nch;
-    {
-        dim3 grid((unsigned)((ngroups + BS_TX - 1) / BS_TX), (unsigned)nblock, (unsigned)g.ndm), block(BS_TX, BS_TY);
-        if (vec4)
-            k_block_sums<4><<<grid, block, 0, st>>>(d_fb, fb_stride_dm, vd, nch, segsum);
-        else
-            k_block_sums<1><<<grid, block, 0, st>>>(d_fb, fb_stride_dm, vd, nch, segsum);
-        cudaError_t e = cudaGetLastError();
-        if (e != cudaSuccess) return e;
-        ++*launches;
-    }
     {
         const long long n = (long long)g.ndm * nch;
         k_channel_stats<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(segsum, (int)nblock, nch, g.ndm, (double)nt, qmean,
@@ -188,6 +203,17 @@ cudaError_t launch_redigitize(const Geometry &g, const float *d_fb, long long fb
         ++*launches;
     }
     return cudaSuccess;
+}
+
+cudaError_t launch_redigitize(const Geometry &g, const float *d_fb, long long fb_stride_dm, long long nblock,
+                              double qmean, double qstd, unsigned char *d_codes, long long codes_stride_dm,
+                              float *d_offset, float *d_scale, void *d_workspace, cudaStream_t st, long long *launches)
+{
+    double *segsum = reinterpret_cast<double *>(d_workspace);
+    cudaError_t e = launch_block_sums(g, d_fb, fb_stride_dm, nblock, segsum, st, launches);
+    if (e != cudaSuccess) return e;
+    return launch_stats_quantize(g, d_fb, fb_stride_dm, nblock, qmean, qstd, segsum, d_codes, codes_stride_dm, d_offset,
+                                 d_scale, st, launches);
 }
 
 }  // namespace cdmt

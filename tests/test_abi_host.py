@@ -8,7 +8,7 @@ import re
 import numpy as np
 import pytest
 
-from paper_1607_00909_b200 import synth
+import cdmt_synth as synth
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
@@ -156,7 +156,7 @@ def test_execute_rejects_null_pointers_before_touching_cuda(cdmt):
     for args in [(0, 16384, 16384, 256, 10 ** 9, 256, 10 ** 9),
                  (256, 16384, 16384, 0, 10 ** 9, 256, 10 ** 9),
                  (256, 16384, 16384, 256, 10 ** 9, 0, 10 ** 9),
-                 (264, 16384, 16384, 256, 10 ** 9, 256, 10 ** 9)]:      # misaligned input
+                 (260, 16384, 16384, 256, 10 ** 9, 256, 10 ** 9)]:      # input not aligned to one complex word
         with pytest.raises(cdmt.CdmtError) as e:
             cdmt.cdmt_execute(p, args[0], args[1], args[2], args[3], args[4], args[5], args[6], stream=0)
         assert e.value.status == cdmt.ERR_ARG

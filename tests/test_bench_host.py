@@ -12,7 +12,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 sys.path.insert(0, ROOT)
 
 import bench  # noqa: E402
-from paper_1607_00909_b200 import synth  # noqa: E402
+import cdmt_synth as synth  # noqa: E402
 
 
 def test_flop_accounting_matches_scope_table():
@@ -42,7 +42,7 @@ import os, sys, json
 sys.path.insert(0, %(root)r)
 import torch, torch.distributed as dist
 import bench
-from paper_1607_00909_b200 import synth
+import cdmt_synth as synth
 dist.init_process_group("gloo")
 rank, world = dist.get_rank(), dist.get_world_size()
 cfg = bench.rank_workload(synth.make_config("c1"), rank, world)

@@ -16,7 +16,7 @@ pytestmark = pytest.mark.gpu
 torch = pytest.importorskip("torch")
 
 from oracle import cdmt_oracle as orc            # noqa: E402
-from paper_1607_00909_b200 import synth          # noqa: E402
+import cdmt_synth as synth          # noqa: E402
 
 
 @pytest.fixture(scope="module")

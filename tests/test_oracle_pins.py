@@ -9,7 +9,7 @@ import numpy as np
 import pytest
 
 from oracle import cdmt_oracle as orc
-from paper_1607_00909_b200 import synth
+import cdmt_synth as synth
 
 GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "paper_values.txt")
 
