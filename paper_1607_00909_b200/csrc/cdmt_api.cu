@@ -234,6 +234,13 @@ static long long chunk_units_for(const cdmt_plan *p, long long nunits)
     const long long cap = ((1LL << 31) - 1) / p->g.nchan / 2;
     if (c > cap) c = cap;
     if (c > nunits) c = nunits;
+    // whole blocks -- and an even number of them -- let the warp-specialised kernel pair the blocks of a
+    // (subband, channel); a caller's explicit CDMT_OPT_CHUNK_UNITS is taken as it is
+    if (p->chunk_units <= 0) {
+        const long long S = p->g.nsub;
+        if (c >= 2 * S) c -= c % (2 * S);
+        else if (c >= S) c -= c % S;
+    }
     return c < 1 ? 1 : c;
 }
 

@@ -418,10 +418,11 @@ cudaError_t launch_fused(const Geometry &g, const Workspace &ws, const float2 *s
     fa.scale = (float)(1.0 / ((double)g.nfft * (double)M));
     fa.dm_first = 0;
     fa.dm_param0 = 0;
+    fa.nb_chunk = 0;
     int logd = 0;
     while ((1 << logd) < D) ++logd;
     // force_generic carries CDMT_OPT_FUSED_KERNEL: 0 auto, 1 generic, 2 scalar fast, 3 packed halves (x2),
-    // 5 packed pols, software-pipelined chirp (sp)
+    // 4 packed halves, warp-specialised, two blocks per CTA (ws), 5 packed pols, software-pipelined chirp (sp)
     const bool fast_ok = !accurate && M >= 512 && D <= 32 && (1 << logd) == D && (g.hdisc % D) == 0 &&
                          poly_phase_ok(g, h_dm, h_fcen);
     // x2 and sp reduce the phase mod 1 with a 2^20 magic number: |phase| must stay below 2^19 cycles
@@ -429,11 +430,13 @@ cudaError_t launch_fused(const Geometry &g, const Workspace &ws, const float2 *s
     const bool x2_ok = fast_ok && small_phase && fused_x2_supported(M, D, g.hdisc);
     const bool sp_ok = fast_ok && small_phase && fused_sp_supported(M, D, g.hdisc);
     if (force_generic == 5 && !sp_ok) return cudaErrorInvalidValue;
-    if (force_generic == 4) return cudaErrorInvalidValue;
+    const bool ws_ok = x2_ok && fused_ws_supported(M, D, g.hdisc, g.nsub, unit0, nunits);
+    if (force_generic == 4 && !ws_ok) return cudaErrorInvalidValue;
     if (force_generic == 3 && !x2_ok) return cudaErrorInvalidValue;
     if (force_generic == 2 && !fast_ok) return cudaErrorInvalidValue;
     // automatic choice: x2 (measured fastest on all five configs: c3 21.8 ms per launch against 22.2 for sp),
     // then sp (covers ndec < 8)
+    if (ws_ok && (force_generic == 0 || force_generic == 4)) return launch_fused_ws(M, logd, fa, h_dm, nunits, st, launches);
     if (x2_ok && (force_generic == 0 || force_generic == 3)) return launch_fused_x2(M, logd, fa, h_dm, nunits, st, launches);
     if (sp_ok && (force_generic == 0 || force_generic == 5)) return launch_fused_sp(M, logd, fa, h_dm, nunits, st, launches);
     const bool fast = fast_ok && force_generic != 1;

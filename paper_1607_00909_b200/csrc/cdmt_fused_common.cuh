@@ -48,6 +48,7 @@ struct FusedArgs {
     long long out_stride_dm;
     int unit0, nsub, nchan, nfft, hdisc, ndec, vdec, ndm, dm_tile, chirp_ref, accurate;
     int dm_first, dm_param0;  // DM range [dm_first, ndm) of this launch; dmp.dm[0] is trial dm_param0
+    int nb_chunk;             // k_fused_ws: whole blocks in this chunk (units = nb_chunk * nsub)
     double bw_mhz;
     float scale;
 };
@@ -110,6 +111,11 @@ __device__ __forceinline__ void lane_reduce_scatter(float *a, int lane)
 bool fused_x2_supported(int M, int ndec, int hdisc);
 cudaError_t launch_fused_x2(int M, int logd, const FusedArgs &fa, const double *h_dm, int nunits, cudaStream_t st,
                             long long *launches);
+// cdmt_fused5.cu
+bool fused_ws_supported(int M, int ndec, int hdisc, int nsub, int unit0, int nunits);
+cudaError_t launch_fused_ws(int M, int logd, const FusedArgs &fa, const double *h_dm, int nunits, cudaStream_t st,
+                            long long *launches);
+
 // cdmt_fused4.cu
 bool fused_sp_supported(int M, int ndec, int hdisc);
 cudaError_t launch_fused_sp(int M, int logd, const FusedArgs &fa, const double *h_dm, int nunits, cudaStream_t st,

@@ -97,11 +97,11 @@ def compare_units(cfg, got_units, ref_units):
 
 
 def check_pulse_peaks(cfg, units, pulse_units, got_units, ref_units):
-    """north_star: identical peak positions on injected pulses.  For a unit that holds a signal the
-    position of the maximum over (DM trial, time sample) of the power summed over the subband's channels
-    must be the oracle's, wherever the oracle's maximum is clear (top-2 margin > 2e-3 rms).
+    """north_star: identical peak positions on injected pulses.  SURVEY Q17: per DM trial, the position of
+    the first maximum over time of the power summed over the subband's channels must be the oracle's,
+    wherever the oracle's maximum is clear (top-2 margin > 2e-3 x rms of that trial's row).
     Impulse configs: the units holding an impulse; pulse-train config (c3): every sampled unit.
-    Returns the number of units whose peak was compared."""
+    Returns the number of (unit, DM trial) rows whose peak position was compared."""
     idx = {u: i for i, u in enumerate(units)}
     todo = [(s, b) for (s, b, _) in pulse_units]
     if cfg.pulse_train is not None:
@@ -110,10 +110,10 @@ def check_pulse_peaks(cfg, units, pulse_units, got_units, ref_units):
     for (s, b) in todo:
         g = got_units[idx[(s, b)]].sum(-1)             # [dm][q] summed over the subband's channels
         r = ref_units[idx[(s, b)]].sum(-1)
-        flat = np.sort(r.ravel())
-        if flat[-1] - flat[-2] > 2e-3 * np.sqrt(np.mean(r ** 2)):
-            assert np.unravel_index(g.argmax(), g.shape) == np.unravel_index(r.argmax(), r.shape), (s, b)
-            checked += 1
+        top = np.sort(r, axis=1)
+        clear = top[:, -1] - top[:, -2] > 2e-3 * np.sqrt(np.mean(r ** 2, axis=1))
+        assert np.array_equal(g.argmax(axis=1)[clear], r.argmax(axis=1)[clear]), (s, b)
+        checked += int(clear.sum())
     return checked
 
 
@@ -177,7 +177,7 @@ def test_c3_stratified_units_then_redigitize_and_incoherent_at_bench_shape(cdmt)
     got_units = [gpu_unit_slice(out, cfg, s, b) for s, b in units]
     ref = oracle_units(cfg, units, keep)
     compare_units(cfg, got_units, ref)
-    assert check_pulse_peaks(cfg, units, pulse_units, got_units, ref) >= len(units) // 2
+    assert check_pulse_peaks(cfg, units, pulse_units, got_units, ref) >= len(units) * cfg.ndm // 2
     del d_in, ws
 
     # ---- N1 at the bench shape: statistics and codes of three planes against the oracle
@@ -238,7 +238,7 @@ def test_c4_stratified_units(cdmt):
     del out
     ref = oracle_units(cfg, units, keep)
     compare_units(cfg, got_units, ref)
-    assert check_pulse_peaks(cfg, units, pulse_units, got_units, ref) >= cfg.nsub
+    assert check_pulse_peaks(cfg, units, pulse_units, got_units, ref) >= len(pulse_units) * cfg.ndm // 2
 
 
 def test_c5_int8_block_groups(cdmt):
@@ -266,7 +266,7 @@ def test_c5_int8_block_groups(cdmt):
     got_units = [got[u] for u in units]
     ref = oracle_units(cfg, units, keep)
     compare_units(cfg, got_units, ref)
-    assert check_pulse_peaks(cfg, units, pulse_units, got_units, ref) >= 10
+    assert check_pulse_peaks(cfg, units, pulse_units, got_units, ref) >= len(pulse_units) * cfg.ndm // 2
 
 
 def test_subband_reference_mode_c2_sample(cdmt):

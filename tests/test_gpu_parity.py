@@ -140,8 +140,8 @@ X2_SHAPES = [
 @pytest.mark.parametrize("shape", X2_SHAPES)
 @pytest.mark.parametrize("ref", [synth.REF_CHANNEL, synth.REF_SUBBAND])
 def test_fused_kernel_variants(cdmt, shape, ref):
-    """CDMT_OPT_FUSED_KERNEL: software-pipelined packed polarisations (5), packed half transforms (3),
-    scalar fast (2) and general (1) kernels."""
+    """CDMT_OPT_FUSED_KERNEL: software-pipelined packed polarisations (5), warp-specialised packed half
+    transforms with two blocks per CTA (4), packed half transforms (3), scalar fast (2) and general (1)."""
     nsub, nsamp, nfft, noverlap, nchan, ndec = shape
     cfg = synth.small_config(nsub=nsub, nsamp=nsamp, nfft=nfft, noverlap=noverlap, nchan=nchan,
                              ndec=ndec, dm=(0.0, 1.5, -3.5, 41.25, 96.0), f_lo=121.0)
@@ -153,10 +153,19 @@ def test_fused_kernel_variants(cdmt, shape, ref):
         kerns.insert(0, 3)
     if M <= 4096:
         kerns.insert(0, 5)
+    if M == 4096 and ndec >= 8:
+        kerns.append(4)
     for kern in kerns:
         got, _ = gpu_run(cdmt, cfg, x, ref, opts={cdmt.OPT_FUSED_KERNEL: kern})
         worst = check_filterbank(got, want)
         assert worst < TOL, (kern, worst)
+    if 4 in kerns:
+        # kernel 4 pairs the blocks of a chunk: one block per chunk (second FFT group idle), a DM tile that
+        # does not divide ndm, and chunks of two blocks (ragged last chunk where nblock is odd)
+        for opts in ({cdmt.OPT_CHUNK_UNITS: nsub, cdmt.OPT_DM_TILE: 2}, {cdmt.OPT_CHUNK_UNITS: 2 * nsub}):
+            opts[cdmt.OPT_FUSED_KERNEL] = 4
+            got, _ = gpu_run(cdmt, cfg, x, ref, opts=opts)
+            check_filterbank(got, want)
     # a DM tile that does not divide ndm, one unit per chunk
     got, _ = gpu_run(cdmt, cfg, x, ref, opts={cdmt.OPT_FUSED_KERNEL: kerns[0], cdmt.OPT_DM_TILE: 2,
                                              cdmt.OPT_CHUNK_UNITS: 1})
@@ -317,7 +326,7 @@ def test_execute_sums_are_the_block_sums_of_the_stored_filterbank(cdmt):
                              dm=(0.0, 1.5, 40.0), f_lo=121.0)
     x = synth.generate(cfg)
     d_in = torch.from_numpy(x).cuda()
-    for kern in (0, 1, 2, 3, 5):
+    for kern in (0, 1, 2, 3, 4, 5):
         plan = cdmt.cdmt_plan_create(**cfg.plan_kwargs())
         cdmt.cdmt_plan_set_option(plan, cdmt.OPT_FUSED_KERNEL, kern)
         q = cdmt.cdmt_plan_query(plan, cfg.nsamp)
@@ -377,7 +386,7 @@ def test_errors_are_codes_not_crashes(cdmt):
 
 
 # ---------------------------------------------------------------- repeatability (stands in for racecheck)
-@pytest.mark.parametrize("kern", [3, 5])
+@pytest.mark.parametrize("kern", [4, 3, 5])
 def test_fused_kernels_are_bit_reproducible(cdmt, kern):
     """compute-sanitizer's racecheck is not available on the GPU pool.  The fused kernels exchange data
     through shared memory under split mbarriers; a missing wait would show as run-to-run differences.
