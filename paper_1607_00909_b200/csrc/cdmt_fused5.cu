@@ -16,7 +16,7 @@
 //    consumers; two buffers, full/empty mbarriers) without touching shared memory.  The FP64 and
 //    XU pipes now run beside the FP32 pipe instead of in turn with it, and the chirp is computed
 //    once per two blocks.  `setmaxnreg` moves the registers the chirp warps do not need to the
-//    FFT warps (96 / 208).
+//    FFT warps (104 / 200 of the 3 x 168 the CTA is launched with).
 //  * An FFT group never waits at its block barrier: the two polarisations have their own
 //    exchange buffers and their own mbarriers, and are staggered --
 //        pass 0 (X * H, radix 16) pol 0, pol 1 | pass 1 pol 0, arrive A0 | pass 1 pol 1, arrive A1
@@ -41,7 +41,8 @@ struct WS {
     static constexpr int R2 = L / 256;     // radix of the last pass
     static constexpr int U2 = 16 / R2;     // last-pass butterflies per thread
     static constexpr int NWARP = NT / 32;  // warps per group (4)
-    static constexpr int NTHREADS = 3 * NT;
+    static constexpr int NGRP = 2;         // FFT groups (blocks) per CTA
+    static constexpr int NTHREADS = (NGRP + 1) * NT;
     static constexpr int PITCH = 17;       // float4 per d1 row: conflict-free 16-byte accesses
     static constexpr int RHO = 16 * PITCH; // float4 per j2 plane
     static constexpr int EX = R2 * RHO;    // float4 per exchange buffer (one per polarisation and group)
@@ -51,7 +52,7 @@ struct WS {
     static constexpr int NBAR = 8 + 16;    // per group A0 A1 F0 F1; per quadrant full[2] empty[2]
     static constexpr size_t group_bytes = sizeof(float4) * 2 * EX + sizeof(float2) * NWARP * INTEG;
     static constexpr size_t smem_bytes = 2 * group_bytes + sizeof(uint64_t) * NBAR + 16;
-    static constexpr int REGS_FFT = 208, REGS_CHIRP = 96;
+    static constexpr int REGS_FFT = 200, REGS_CHIRP = 104;  // 2 x 200 + 104 = 3 x 168: what the CTA holds at launch
 };
 
 __device__ __forceinline__ unsigned ws_f2u(float x) { return __float_as_uint(x); }
@@ -91,7 +92,7 @@ k_fused_ws(const FusedArgs a, const __grid_constant__ DmParams dmp)
     uint32_t *tslot = reinterpret_cast<uint32_t *>(bars + G::NBAR);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int role = warp >> 2;          // 0, 1: FFT group A, B; 2: chirp warps
+    const int role = warp >> 2;          // 0, 1: FFT group A, B; NGRP: chirp warps
     const int q = warp & 3;              // TMEM lane quadrant
     const int t = tid & (NT - 1);        // thread index inside the role: the same bins in all three
     const int c = blockIdx.x % a.nchan;
@@ -119,7 +120,7 @@ k_fused_ws(const FusedArgs a, const __grid_constant__ DmParams dmp)
     const int j1 = t & 15, j2 = t >> 4;      // pass-0 role; pass 1: (j2, t0 = t & 15)
     const int rest = j1 * R2 + j2;           // half-transform input index j = j0 L/16 + rest
 
-    if (role == 2) {
+    if (role == G::NGRP) {
         // ------------------------------------------------------------------ chirp warps
         {
             // pass twiddles of thread t: w1[r] = exp(2 pi i r t0 / 256), w2[u][r] = exp(2 pi i r beta_u / L)
@@ -255,112 +256,14 @@ k_fused_ws(const FusedArgs a, const __grid_constant__ DmParams dmp)
             const int nchan_total = a.nsub * a.nchan;
             const int ochan = nchan_total - 1 - (s * a.nchan + c);
             float *out0 = a.out + (size_t)b * a.vdec * nchan_total + ochan;
-#pragma unroll 1
-            for (int d = d_begin; d < d_end; ++d) {
-                const unsigned i = (unsigned)(d - d_begin), buf = i & 1u, par = i & 1u;
-                // ---- H(d) from the chirp warp
-                P2 Hr[16], Hi[16];
-                {
-                    mbar_wait(full + buf, (i >> 1) & 1u);
-                    tmem_fence_after_sync();
-                    unsigned h[64];
-                    tmem_ld64(h, tcol + G::COL_H + 64 * buf);
-#pragma unroll
-                    for (int r = 0; r < 16; ++r) {
-                        Hr[r] = ws_pku(h[4 * r], h[4 * r + 1]);
-                        Hi[r] = ws_pku(h[4 * r + 2], h[4 * r + 3]);
-                    }
-                }
-                // ---- pass 0, both polarisations (a buffer is free once every thread of the group has
-                //      taken its pass-2 loads of the previous trial)
-#pragma unroll
-                for (int pol = 0; pol < 2; ++pol) {
-                    unsigned xr[64];
-                    tmem_ld64(xr, tX + 64 * pol);
-                    C2 v[16];
-#pragma unroll
-                    for (int r = 0; r < 16; ++r)
-                        v[r] = cmulp(C2{ws_pku(xr[4 * r], xr[4 * r + 1]), ws_pku(xr[4 * r + 2], xr[4 * r + 3])}, Hr[r], Hi[r]);
-                    PDft<16>::run(v);
-                    if (i != 0u) mbar_wait(pol ? barF1 : barF0, par ^ 1u);
-                    float4 *dst = (pol ? ex1 : ex0) + j2 * G::RHO + j1 * G::PITCH;
-#pragma unroll
-                    for (int t0 = 0; t0 < 16; ++t0) dst[t0] = ws_c2_to_f4(v[t0]);
-                }
-                ws_warp_arrive(empty + buf, lane);  // H(d) consumed (also orders the half-warp exchange below)
-                // ---- pass 1: along j1, in place, half-warp local
-                {
-                    unsigned w1[32];
-                    tmem_ld32(w1, tcol + G::COL_TW1);
-#pragma unroll
-                    for (int pol = 0; pol < 2; ++pol) {
-                        float4 *p = (pol ? ex1 : ex0) + j2 * G::RHO + (t & 15);
-                        C2 v[16];
-#pragma unroll
-                        for (int d1 = 0; d1 < 16; ++d1) v[d1] = ws_f4_to_c2(p[d1 * G::PITCH]);
-#pragma unroll
-                        for (int d1 = 1; d1 < 16; ++d1) v[d1] = cmuls(v[d1], ws_u2f(w1[2 * d1]), ws_u2f(w1[2 * d1 + 1]));
-                        PDft<16>::run(v);
-#pragma unroll
-                        for (int t1 = 0; t1 < 16; ++t1) p[t1 * G::PITCH] = ws_c2_to_f4(v[t1]);
-                        mbar_arrive(pol ? barA1 : barA0);
-                    }
-                }
-                // ---- pass 2 along j2, radix-2 combine, detection, polarisation sum
-                P2 pw[16];  // (|y[t']|^2, |y[t' + L]|^2) summed over polarisations, order k = u R2 + t2
-                {
-                    unsigned w2[32];
-                    tmem_ld32(w2, tcol + G::COL_TW2);
-#pragma unroll
-                    for (int pol = 0; pol < 2; ++pol) {
-                        const float4 *ex = pol ? ex1 : ex0;
-                        mbar_wait(pol ? barA1 : barA0, par);
-                        C2 v[16];
-#pragma unroll
-                        for (int u = 0; u < U2; ++u) {
-                            const int beta = t + NT * u;
-                            const float4 *p = ex + (beta >> 4) * G::PITCH + (beta & 15);
-#pragma unroll
-                            for (int rr = 0; rr < R2; ++rr) v[u * R2 + rr] = ws_f4_to_c2(p[rr * G::RHO]);
-                        }
-#pragma unroll
-                        for (int u = 0; u < U2; ++u) {
-#pragma unroll
-                            for (int rr = 1; rr < R2; ++rr)
-                                v[u * R2 + rr] = cmuls(v[u * R2 + rr], ws_u2f(w2[2 * (u * R2 + rr)]), ws_u2f(w2[2 * (u * R2 + rr) + 1]));
-                        }
-                        mbar_arrive(pol ? barF1 : barF0);  // this thread's loads of the trial have been consumed
-#pragma unroll
-                        for (int u = 0; u < U2; ++u) PDft<R2>::run(v + u * R2);
-#pragma unroll
-                        for (int h = 0; h < 2; ++h) {
-                            unsigned wf[32];
-                            tmem_ld32(wf, tcol + G::COL_TWF + 32 * h);
-#pragma unroll
-                            for (int kk = 0; kk < 8; ++kk) {
-                                const int k = 8 * h + kk;
-                                const P2 Wr = ws_pku(wf[4 * kk], wf[4 * kk + 1]), Wi = ws_pku(wf[4 * kk + 2], wf[4 * kk + 3]);
-                                const P2 re = v[k].re, im = v[k].im;  // lanes (A, B)
-                                const P2 yr = fma2(ws_hi2(im), neg2(Wi), fma2(ws_hi2(re), Wr, ws_lo2(re)));
-                                const P2 yi = fma2(ws_hi2(re), Wi, fma2(ws_hi2(im), Wr, ws_lo2(im)));
-                                pw[k] = pol ? fma2(yi, yi, fma2(yr, yr, pw[k])) : fma2(yi, yi, mul2(yr, yr));
-                            }
-                        }
-                    }
-                }
-                // ---- time integration over D adjacent samples = D adjacent lanes
-                __syncwarp();  // the previous trial's reads of this warp's tile are done
-#pragma unroll
-                for (int k = 0; k < 16; ++k) {
-                    const int n = (k / R2) + U2 * (k % R2);
-                    float2 v2;
-                    upk(pw[k], v2.x, v2.y);
-                    ib[n * G::IROW + lane] = v2;
-                }
-                __syncwarp();
-                float *outd = out0 + (size_t)d * (size_t)a.out_stride_dm;
-                const int il = lane & (DG - 1), g0 = lane - il;
-                const int tgrp = (D > 16) ? (t & ~31) : (t - il);  // first sample of the group, before + NT n
+            const int il = lane & (DG - 1), g0 = lane - il;
+            const int tgrp = (D > 16) ? (t & ~31) : (t - il);  // first sample of a lane's group, before + NT n
+
+            // Second half of the time integration of one trial (the tile was filled at the end of that
+            // trial): one lane sums the D adjacent samples of a row, scales and stores them time-major.
+            // It runs inside the NEXT trial, where its shared-memory and store latencies are covered.
+            auto integrate_store = [&](int dd) {
+                float *outd = out0 + (size_t)dd * (size_t)a.out_stride_dm;
 #pragma unroll
                 for (int kk = 0; kk < 16 / DG; ++kk) {
                     const int n = il + DG * kk;
@@ -384,7 +287,134 @@ k_fused_ws(const FusedArgs a, const __grid_constant__ DmParams dmp)
                         if (t1 >= a.hdisc && t1 < M - a.hdisc) outd[(size_t)((t1 - a.hdisc) >> LOGD) * nchan_total] = s1 * a.scale;
                     }
                 }
+            };
+
+#pragma unroll 1
+            for (int d = d_begin; d < d_end; ++d) {
+                const unsigned i = (unsigned)(d - d_begin), buf = i & 1u, par = i & 1u;
+                const uint32_t tH = tcol + G::COL_H + 64 * buf;
+                // ---- pass 0: Z = X * H(d), radix 16 over j0, both polarisations.  X and H come from TMEM in
+                //      pieces of four bins, the next piece in flight while this one is multiplied.
+                mbar_wait(full + buf, (i >> 1) & 1u);  // H(d) written by the chirp warp
+                tmem_fence_after_sync();
+                unsigned hq[2][16], xq[2][16];
+                tmem_ld16_async(hq[0], tH);
+                tmem_ld16_async(xq[0], tX);
+#pragma unroll
+                for (int pol = 0; pol < 2; ++pol) {
+                    C2 v[16];
+#pragma unroll
+                    for (int cq = 0; cq < 4; ++cq) {
+                        const int cur = cq & 1, nxt = cur ^ 1;
+                        tmem_ld_wait();
+                        tmem_regs16(hq[cur]);
+                        tmem_regs16(xq[cur]);
+                        if (cq < 3 || pol == 0) {
+                            const int pn = cq < 3 ? pol : 1, cn = cq < 3 ? cq + 1 : 0;
+                            tmem_ld16_async(hq[nxt], tH + 16 * cn);
+                            tmem_ld16_async(xq[nxt], tX + 64 * pn + 16 * cn);
+                        }
+#pragma unroll
+                        for (int rr = 0; rr < 4; ++rr) {
+                            const int r = 4 * cq + rr;
+                            v[r] = cmulp(C2{ws_pku(xq[cur][4 * rr], xq[cur][4 * rr + 1]), ws_pku(xq[cur][4 * rr + 2], xq[cur][4 * rr + 3])},
+                                         ws_pku(hq[cur][4 * rr], hq[cur][4 * rr + 1]), ws_pku(hq[cur][4 * rr + 2], hq[cur][4 * rr + 3]));
+                        }
+                    }
+                    if (pol == 0 && i != 0u) integrate_store(d - 1);  // the tile of the previous trial
+                    PDft<16>::run(v);
+                    if (i != 0u) mbar_wait(pol ? barF1 : barF0, par ^ 1u);  // pass-2 loads of trial d-1 are done
+                    float4 *dst = (pol ? ex1 : ex0) + j2 * G::RHO + j1 * G::PITCH;
+#pragma unroll
+                    for (int t0 = 0; t0 < 16; ++t0) dst[t0] = ws_c2_to_f4(v[t0]);
+                }
+                ws_warp_arrive(empty + buf, lane);  // H(d) consumed; also orders the half-warp exchange below
+                // ---- pass 1: along j1, in place, half-warp local; both polarisations' loads up front
+                unsigned w2[32];
+                {
+                    unsigned w1[32];
+                    tmem_ld32_async(w1, tcol + G::COL_TW1);
+                    float4 *p0 = ex0 + j2 * G::RHO + (t & 15), *p1 = ex1 + j2 * G::RHO + (t & 15);
+                    C2 v0[16], v1[16];
+#pragma unroll
+                    for (int d1 = 0; d1 < 16; ++d1) v0[d1] = ws_f4_to_c2(p0[d1 * G::PITCH]);
+#pragma unroll
+                    for (int d1 = 0; d1 < 16; ++d1) v1[d1] = ws_f4_to_c2(p1[d1 * G::PITCH]);
+                    tmem_ld_wait();
+                    tmem_regs32(w1);
+#pragma unroll
+                    for (int d1 = 1; d1 < 16; ++d1) v0[d1] = cmuls(v0[d1], ws_u2f(w1[2 * d1]), ws_u2f(w1[2 * d1 + 1]));
+                    PDft<16>::run(v0);
+#pragma unroll
+                    for (int t1 = 0; t1 < 16; ++t1) p0[t1 * G::PITCH] = ws_c2_to_f4(v0[t1]);
+                    mbar_arrive(barA0);
+#pragma unroll
+                    for (int d1 = 1; d1 < 16; ++d1) v1[d1] = cmuls(v1[d1], ws_u2f(w1[2 * d1]), ws_u2f(w1[2 * d1 + 1]));
+                    tmem_ld32_async(w2, tcol + G::COL_TW2);  // for pass 2, in flight during this butterfly
+                    PDft<16>::run(v1);
+#pragma unroll
+                    for (int t1 = 0; t1 < 16; ++t1) p1[t1 * G::PITCH] = ws_c2_to_f4(v1[t1]);
+                    mbar_arrive(barA1);
+                }
+                // ---- pass 2 along j2, radix-2 combine, detection, polarisation sum
+                P2 pw[16];  // (|y[t']|^2, |y[t' + L]|^2) summed over polarisations, order k = u R2 + t2
+#pragma unroll
+                for (int pol = 0; pol < 2; ++pol) {
+                    const float4 *ex = pol ? ex1 : ex0;
+                    mbar_wait(pol ? barA1 : barA0, par);
+                    C2 v[16];
+#pragma unroll
+                    for (int u = 0; u < U2; ++u) {
+                        const int beta = t + NT * u;
+                        const float4 *p = ex + (beta >> 4) * G::PITCH + (beta & 15);
+#pragma unroll
+                        for (int rr = 0; rr < R2; ++rr) v[u * R2 + rr] = ws_f4_to_c2(p[rr * G::RHO]);
+                    }
+                    if (pol == 0) {
+                        tmem_ld_wait();
+                        tmem_regs32(w2);
+                    }
+                    unsigned wf[2][16];
+                    tmem_ld16_async(wf[0], tcol + G::COL_TWF);
+#pragma unroll
+                    for (int u = 0; u < U2; ++u) {
+#pragma unroll
+                        for (int rr = 1; rr < R2; ++rr)
+                            v[u * R2 + rr] = cmuls(v[u * R2 + rr], ws_u2f(w2[2 * (u * R2 + rr)]), ws_u2f(w2[2 * (u * R2 + rr) + 1]));
+                    }
+                    mbar_arrive(pol ? barF1 : barF0);  // this thread's loads of the trial have been consumed
+#pragma unroll
+                    for (int u = 0; u < U2; ++u) PDft<R2>::run(v + u * R2);
+#pragma unroll
+                    for (int cq = 0; cq < 4; ++cq) {
+                        const int cur = cq & 1, nxt = cur ^ 1;
+                        tmem_ld_wait();
+                        tmem_regs16(wf[cur]);
+                        if (cq < 3) tmem_ld16_async(wf[nxt], tcol + G::COL_TWF + 16 * (cq + 1));
+#pragma unroll
+                        for (int kk = 0; kk < 4; ++kk) {
+                            const int k = 4 * cq + kk;
+                            const P2 Wr = ws_pku(wf[cur][4 * kk], wf[cur][4 * kk + 1]), Wi = ws_pku(wf[cur][4 * kk + 2], wf[cur][4 * kk + 3]);
+                            const P2 re = v[k].re, im = v[k].im;  // lanes (A, B)
+                            const P2 yr = fma2(ws_hi2(im), neg2(Wi), fma2(ws_hi2(re), Wr, ws_lo2(re)));
+                            const P2 yi = fma2(ws_hi2(re), Wi, fma2(ws_hi2(im), Wr, ws_lo2(im)));
+                            pw[k] = pol ? fma2(yi, yi, fma2(yr, yr, pw[k])) : fma2(yi, yi, mul2(yr, yr));
+                        }
+                    }
+                }
+                // ---- first half of the time integration: the 32 powers of this thread (times t + NT n [+ L])
+                //      go to the warp's tile so that D adjacent samples meet in one lane
+                __syncwarp();  // the reads of the previous trial's tile are done
+#pragma unroll
+                for (int k = 0; k < 16; ++k) {
+                    const int n = (k / R2) + U2 * (k % R2);
+                    float2 v2;
+                    upk(pw[k], v2.x, v2.y);
+                    ib[n * G::IROW + lane] = v2;
+                }
+                __syncwarp();
             }
+            if (d_begin < d_end) integrate_store(d_end - 1);
         }
     }
     tmem_fence_before_sync();
