@@ -371,39 +371,68 @@ def main():
                 "share_of_step": prof["ms_fused"] / ms,
                 "forward_fft_ms_per_step": prof["ms_forward"] / args.steps}
 
-    # ---- extra (not part of `value`): 8-bit redigitisation of the filterbanks just computed
-    # (Alg. 1 l.104-106); HBM bound: 4 + 4 bytes read and 1 byte written per filterbank sample
+    # ---- extra (not part of `value`): Alg. 1 l.104-106, 8-bit redigitisation of the filterbanks.  The block
+    # sums come out of the fused kernel (cdmt_execute_sums), so the redigitisation proper reads the float32
+    # filterbank once: 4 bytes read + 1 byte written per sample.  Timed on the last block group of the step
+    # (the whole observation when the output is resident), and the whole device path with 8-bit output.
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm = float(peaks.get("hbm_gbs", 0)) or None
     redig = None
-    if not args.no_redigitize and groups == 1:
+    if not args.no_redigitize:
         try:
-            nws = cdmt.cdmt_redigitize_workspace_bytes(plan, nb_total)
-            d_codes = torch.empty((cfg.ndm, nt, nch), dtype=torch.uint8, device=dev)
+            nb_last = nb_total - (groups - 1) * nb_group
+            b0_last = (groups - 1) * nb_group
+            nws = cdmt.cdmt_redigitize_workspace_bytes(plan, nb_group)
+            d_codes = torch.empty((cfg.ndm, nb_group * cfg.nvalid_dec, nch), dtype=torch.uint8, device=dev)
             d_off = torch.empty((cfg.ndm, nch), dtype=torch.float32, device=dev)
             d_sc = torch.empty((cfg.ndm, nch), dtype=torch.float32, device=dev)
-            d_rws = torch.empty(nws, dtype=torch.uint8, device=dev)
+            d_sums = torch.empty(nws // 8, dtype=torch.float64, device=dev)
+            esz = 2 if int8 else 8
+
+            def group_8bit(b0, nb):
+                ns = (nb - 1) * cfg.step + cfg.nfft
+                cdmt.cdmt_execute_sums(plan, d_in.data_ptr() + b0 * cfg.step * esz, ns, cfg.nsamp, out, out[0].numel(),
+                                       d_sums, ws, ws.numel(), stream)
+                cdmt.cdmt_redigitize_sums(plan, out, out[0].numel(), nb, 64.0, 16.0, d_sums, d_codes,
+                                          d_codes[0].numel(), d_off, d_sc, stream)
+
+            group_8bit(b0_last, nb_last)          # leaves the last group's filterbank and sums in place
             r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             reps = 3
-            for i in range(reps + 1):
-                if i == 1:
-                    r0.record(stream)
-                cdmt.cdmt_redigitize(plan, out, out[0].numel(), nb_total, 64.0, 16.0, d_codes, d_codes[0].numel(),
-                                     d_off, d_sc, d_rws, nws, stream)
+            r0.record(stream)
+            for _ in range(reps):
+                cdmt.cdmt_redigitize_sums(plan, out, out[0].numel(), nb_last, 64.0, 16.0, d_sums, d_codes,
+                                          d_codes[0].numel(), d_off, d_sc, stream)
             r1.record(stream)
             torch.cuda.synchronize()
             rms = r0.elapsed_time(r1) / reps
-            rbytes = 9.0 * out.numel()
-            peaks = {}
-            try:
-                peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
-            except Exception:
-                pass
-            hbm = float(peaks.get("hbm_gbs", 0)) or None
+            rbytes = 5.0 * cfg.ndm * nb_last * cfg.nvalid_dec * nch
+            # the whole device path with 8-bit output: every group through execute_sums + redigitize_sums
+            s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ksteps = max(1, min(args.steps, 3))
+            s0.record(stream)
+            for _ in range(ksteps):
+                for b0 in range(0, nb_total, nb_group):
+                    group_8bit(b0, min(nb_group, nb_total - b0))
+            s1.record(stream)
+            torch.cuda.synchronize()
+            step8 = s0.elapsed_time(s1) / ksteps
             redig = {"ms_per_call": rms, "bytes": rbytes, "achieved_gbs": rbytes / rms / 1e6,
                      "peak_gbs": hbm, "frac": (rbytes / rms / 1e6 / hbm) if hbm else None,
                      "peak_source": "MEASURED_PEAKS.json hbm_gbs" if hbm else "unavailable",
-                     "launches": int(cdmt.cdmt_last_launch_count(plan)),
-                     "note": "cdmt_redigitize on the step's filterbanks; not included in value"}
-            del d_codes, d_rws
+                     "launches": int(cdmt.cdmt_last_launch_count(plan)), "blocks": int(nb_last),
+                     "step_ms_8bit_output": step8,
+                     "value_8bit_output": whole_job_value(full_cfg, 1, step8 * 1e-3) if strong else
+                                          whole_job_value(cfg, world, step8 * 1e-3),
+                     "note": "cdmt_redigitize_sums (channel statistics + quantisation; block sums taken inside the "
+                             "fused kernel) on the last block group of the step; step_ms_8bit_output = the whole "
+                             "device-resident path with 8-bit output (cdmt_execute_sums + cdmt_redigitize_sums per "
+                             "group); neither is part of `value`"}
+            del d_codes, d_sums
         except Exception as e:   # never lose the headline line to the extra leg
             redig = {"error": str(e)}
 
@@ -443,30 +472,49 @@ def main():
         except Exception as e:
             incoh = {"error": str(e)}
 
-    # ---- end to end through the host-buffer entry point (pinned host memory, copies timed)
+    # ---- end to end through the host-buffer entry point (pinned host memory, copies timed): float32
+    # filterbanks (the output `value` is measured on) and the paper's 8-bit product (Alg. 1 l.104-108)
     e2e = None
+    e2e_u8 = None
     if want_e2e:
         del out
         torch.cuda.empty_cache()
-        h_out = torch.empty((cfg.ndm, nt, nch), dtype=torch.float32).pin_memory()
-        nbytes = cdmt.cdmt_host_scratch_bytes(plan, cfg.nsamp)
-        d_scr = torch.empty(nbytes, dtype=torch.uint8, device=dev)
-        cdmt.cdmt_execute_host(plan, h_in.data_ptr(), cfg.nsamp, cfg.nsamp, h_out.data_ptr(), d_scr, nbytes, stream)
         ksteps = max(1, min(args.steps, 3))
-        barrier()
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        for _ in range(ksteps):
-            cdmt.cdmt_execute_host(plan, h_in.data_ptr(), cfg.nsamp, cfg.nsamp, h_out.data_ptr(), d_scr, nbytes, stream)
-        torch.cuda.synchronize()
-        dt = (time.perf_counter() - t0) / ksteps
-        dt = max_over_ranks(dt, world, dev)
-        h2d_b, d2h_b = cdmt.cdmt_host_traffic_bytes(plan, cfg.nsamp)
-        e2e = {"value": whole_job_value(full_cfg, 1, dt) if strong else whole_job_value(cfg, world, dt), "unit": UNIT,
-               "h2d_bytes_per_step": int(h2d_b), "d2h_bytes_per_step": int(d2h_b),
-               "ms_per_step": dt * 1e3, "steps": ksteps,
-               "api": "cdmt_execute_host (pinned host in/out, double-buffered copy streams)"}
-        del d_scr
+
+        def host_leg(kind):
+            lay = cdmt.cdmt_host_layout(plan, cfg.nsamp, kind)
+            u8 = kind == cdmt.OUT_U8
+            h_out = torch.empty((cfg.ndm, nt, nch), dtype=torch.uint8 if u8 else torch.float32).pin_memory()
+            h_off = torch.empty((lay["ngroups"], cfg.ndm, nch), dtype=torch.float32).pin_memory() if u8 else None
+            h_sc = torch.empty((lay["ngroups"], cfg.ndm, nch), dtype=torch.float32).pin_memory() if u8 else None
+            d_scr = torch.empty(lay["scratch_bytes"], dtype=torch.uint8, device=dev)
+
+            def call():
+                cdmt.cdmt_execute_host_async(plan, h_in.data_ptr(), cfg.nsamp, cfg.nsamp, kind, h_out.data_ptr(),
+                                             h_off.data_ptr() if u8 else 0, h_sc.data_ptr() if u8 else 0, 64.0, 16.0,
+                                             d_scr, d_scr.numel(), stream)
+                stream.synchronize()
+            call()
+            barrier()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            for _ in range(ksteps):
+                call()
+            torch.cuda.synchronize()
+            dt = (time.perf_counter() - t0) / ksteps
+            dt = max_over_ranks(dt, world, dev)
+            return {"value": whole_job_value(full_cfg, 1, dt) if strong else whole_job_value(cfg, world, dt),
+                    "unit": UNIT, "h2d_bytes_per_step": int(lay["h2d_bytes"]), "d2h_bytes_per_step": int(lay["d2h_bytes"]),
+                    "ms_per_step": dt * 1e3, "steps": ksteps, "groups": lay["ngroups"],
+                    "api": "cdmt_execute_host_async(%s) + stream synchronize (pinned host in/out, double-buffered "
+                           "copy streams)" % ("CDMT_OUT_U8" if u8 else "CDMT_OUT_F32")}
+
+        e2e = host_leg(cdmt.OUT_F32)
+        torch.cuda.empty_cache()
+        try:
+            e2e_u8 = host_leg(cdmt.OUT_U8)
+        except Exception as e:
+            e2e_u8 = {"error": str(e)}
 
     # ---- CPU baseline: the oracle, as it stands, on a bounded sample (rank 0, N=1 only)
     cpu = None
@@ -487,7 +535,7 @@ def main():
             "scaling": "strong" if strong else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": workload_config(full_cfg if strong else cfg, args),
             "real_time_factor": cfg.nsamp * synth.TSAMP_S / sec_per_step,
-            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+            "clocks": clocks, "e2e": e2e, "e2e_8bit_output": e2e_u8, "gpu_launches": int(launches),
             "roofline": roofline, "cpu_baseline": cpu, "redigitize": redig, "incoherent": incoh,
             "gen_seconds": t_gen, "out_groups": groups,
         }

@@ -68,7 +68,7 @@ enum {
                                   (chirp of the next trial formed in the shadow of the block barrier); 2 to 5
                                   make cdmt_execute fail with CDMT_ERR_CUDA where they do not apply */
     CDMT_OPT_FORCE_GENERIC = 4, /* older name of the same key (value 1) */
-    CDMT_OPT_HOST_GROUP_BLOCKS = 5, /* cdmt_execute_host: blocks staged per group (0 = about 512 MiB of output) */
+    CDMT_OPT_HOST_GROUP_BLOCKS = 5, /* cdmt_execute_host: blocks staged per group (0 = about 1 GiB of output, an even number) */
     CDMT_OPT_KEEP_TABLES = 6  /* 1: the caller promises that nothing but this plan's executes writes to
                                  d_workspace between calls that pass the same workspace pointer; the DM list,
                                  centre frequencies and twiddle tables at its head are then written by the

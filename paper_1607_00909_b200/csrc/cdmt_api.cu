@@ -332,11 +332,13 @@ static int run_chunks(cdmt_plan *plan, const void *d_in, long long in_stride_pol
         if (!mark(&b)) return check_cuda(cudaErrorUnknown);
         if (profile) plan->spans.push_back({a, b, 0});
         if (d_out) {
+            bool chunk_sums = true;
             rc = check_cuda(launch_fused(g, ws, spec, (int)u0, n, d_out, out_stride_dm, plan->dm_tile,
                                          plan->accurate, plan->force_generic, plan->dm.data(),
-                                         plan->fcen.data(), d_segsum, (int)nb, &sums_done, st,
+                                         plan->fcen.data(), d_segsum, (int)nb, &chunk_sums, st,
                                          &plan->last_launches));
             if (rc) return rc;
+            sums_done = sums_done && chunk_sums;
             if (!mark(&c)) return check_cuda(cudaErrorUnknown);
             if (profile) plan->spans.push_back({b, c, 1});
         }
@@ -439,12 +441,15 @@ extern "C" int cdmt_unpack(cdmt_plan *plan, const void *d_in, long long nsamp, l
 // output staging buffers are doubled: the host-to-device copy of group i+1 and the
 // device-to-host copy of group i-1 run on their own streams while group i computes.
 
-// blocks per staged group: keep the staged output near 512 MiB
+// blocks per staged group: keep the staged output near 1 GiB, and the number of blocks even (the
+// warp-specialised fused kernel works on pairs of blocks)
 static long long host_group_blocks(const cdmt_plan *plan, long long nb)
 {
     const Geometry &g = plan->g;
     const long long per_block = (long long)g.ndm * g.vdec * g.nsub * g.nchan * (long long)sizeof(float);
-    long long gb = (1LL << 29) / (per_block > 0 ? per_block : 1);
+    long long gb = (1LL << 30) / (per_block > 0 ? per_block : 1);
+    if (gb < 2) gb = 2;
+    gb -= gb & 1;
     if (plan->host_group > 0) gb = plan->host_group;
     if (gb < 1) gb = 1;
     if (gb > nb) gb = nb;

@@ -51,7 +51,11 @@ struct WS {
     static constexpr int COL_XA = 0, COL_TW1 = 256, COL_TW2 = 288, COL_TWF = 320, COL_H = 384;
     static constexpr int NBAR = 8 + 16;    // per group A0 A1 F0 F1; per quadrant full[2] empty[2]
     static constexpr size_t group_bytes = sizeof(float4) * 2 * EX + sizeof(float2) * NWARP * INTEG;
-    static constexpr size_t smem_bytes = 2 * group_bytes + sizeof(uint64_t) * NBAR + 16;
+    // block sums (SUMS): the FFT lanes hand the two values they stored to the chirp warps through
+    // fsum[slot][group][thread] (float4, four trials deep); the chirp warps leave their pairs in psum[parity][group][q]
+    static constexpr int SUM_SLOTS = 4;
+    static constexpr size_t smem_bytes = 2 * group_bytes + sizeof(uint64_t) * NBAR + 16 +
+                                         sizeof(float4) * SUM_SLOTS * NGRP * NT + sizeof(double2) * 2 * NGRP * NWARP;
     static constexpr int REGS_FFT = 200, REGS_CHIRP = 104;  // 2 x 200 + 104 = 3 x 168: what the CTA holds at launch
 };
 
@@ -77,7 +81,7 @@ __device__ __forceinline__ void ws_warp_arrive(uint64_t *bar, int lane)
     if (lane == 0) mbar_arrive(bar);
 }
 
-template <int M, int LOGD>
+template <int M, int LOGD, bool SUMS>
 __global__ void __launch_bounds__(WS<M>::NTHREADS, 1)
 k_fused_ws(const FusedArgs a, const __grid_constant__ DmParams dmp)
 {
@@ -90,6 +94,8 @@ k_fused_ws(const FusedArgs a, const __grid_constant__ DmParams dmp)
     extern __shared__ float4 smem4[];
     uint64_t *bars = reinterpret_cast<uint64_t *>(reinterpret_cast<char *>(smem4) + 2 * G::group_bytes);
     uint32_t *tslot = reinterpret_cast<uint32_t *>(bars + G::NBAR);
+    float4 *fsum = reinterpret_cast<float4 *>(tslot + 4);                                      // [slot][group][NT]
+    double2 *psum = reinterpret_cast<double2 *>(fsum + G::SUM_SLOTS * G::NGRP * NT);             // [parity][group][q]
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int role = warp >> 2;          // 0, 1: FFT group A, B; NGRP: chirp warps
@@ -185,6 +191,35 @@ k_fused_ws(const FusedArgs a, const __grid_constant__ DmParams dmp)
         tmem_fence_before_sync();
         __syncthreads();  // X and twiddles are in TMEM
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(G::REGS_CHIRP));
+        // Block sums of trial index j (Alg. 1 l.104): this warp adds, in fp64, the values the FFT lanes of its
+        // quadrant stored (sum and sum of squares), the four chirp warps meet at a named barrier, and two
+        // threads add the four pairs in quadrant order and write them out.
+        const int nchan_total = a.nsub * a.nchan;
+        const int ochan = nchan_total - 1 - (s * a.nchan + c);
+        auto block_sums = [&](unsigned j) {
+            double2 *ps = psum + (size_t)(j & 1u) * G::NGRP * G::NWARP;
+#pragma unroll
+            for (int g = 0; g < G::NGRP; ++g) {
+                if (g == 1 && !has_b) break;
+                const float4 v = fsum[((size_t)(j & (G::SUM_SLOTS - 1)) * G::NGRP + g) * NT + t];
+                double a1 = ((double)v.x + (double)v.y) + ((double)v.z + (double)v.w);
+                double a2 = fma((double)v.x, (double)v.x, fma((double)v.y, (double)v.y,
+                                fma((double)v.z, (double)v.z, (double)v.w * (double)v.w)));
+                warp_sum_pair(a1, a2);
+                if (lane == 0) ps[g * G::NWARP + q] = make_double2(a1, a2);
+            }
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+            if (t < G::NGRP && (t == 0 || has_b)) {
+                double a1 = 0.0, a2 = 0.0;
+#pragma unroll
+                for (int w = 0; w < G::NWARP; ++w) {
+                    a1 += ps[t * G::NWARP + w].x;
+                    a2 += ps[t * G::NWARP + w].y;
+                }
+                const int b = a.unit0 / a.nsub + 2 * bp + t;
+                a.segsum[((size_t)(d_begin + (int)j) * a.nblock_total + b) * nchan_total + ochan] = make_double2(a1, a2);
+            }
+        };
 #pragma unroll 1
         for (int d = d_begin; d < d_end; ++d) {
             const unsigned i = (unsigned)(d - d_begin), buf = i & 1u;
@@ -219,6 +254,17 @@ k_fused_ws(const FusedArgs a, const __grid_constant__ DmParams dmp)
                 tmem_st16(tcol + G::COL_H + 64 * buf + 16 * part, h);
             }
             ws_warp_arrive(full + buf, lane);
+            // the `empty` wait above ordered this warp after pass 0 of trial i - 2 in both FFT groups, which
+            // comes after they handed over the values of trial i - 3
+            if (SUMS && i >= 3u) block_sums(i - 3u);
+        }
+        if (SUMS) {
+            // the last three trials: after every FFT warp has left its loop
+            tmem_fence_before_sync();
+            __syncthreads();
+            const unsigned n = (unsigned)max(0, d_end - d_begin);
+            for (unsigned j = n > 3u ? n - 3u : 0u; j < n; ++j) block_sums(j);
+            return;
         }
     } else {
         // ------------------------------------------------------------------ FFT groups
@@ -264,6 +310,7 @@ k_fused_ws(const FusedArgs a, const __grid_constant__ DmParams dmp)
             // It runs inside the NEXT trial, where its shared-memory and store latencies are covered.
             auto integrate_store = [&](int dd) {
                 float *outd = out0 + (size_t)dd * (size_t)a.out_stride_dm;
+                float mine[4] = {0.f, 0.f, 0.f, 0.f};  // what this lane stores (two values per kk step)
 #pragma unroll
                 for (int kk = 0; kk < 16 / DG; ++kk) {
                     const int n = il + DG * kk;
@@ -282,11 +329,24 @@ k_fused_ws(const FusedArgs a, const __grid_constant__ DmParams dmp)
                     }
                     const int t0 = tgrp + NT * n;
                     if (D <= 16 || lane < 16) {
-                        if (t0 >= a.hdisc && t0 < M - a.hdisc) outd[(size_t)((t0 - a.hdisc) >> LOGD) * nchan_total] = s0 * a.scale;
+                        if (t0 >= a.hdisc && t0 < M - a.hdisc) {
+                            const float f = s0 * a.scale;
+                            outd[(size_t)((t0 - a.hdisc) >> LOGD) * nchan_total] = f;
+                            mine[(2 * kk) & 3] = f;
+                        }
                         const int t1 = t0 + L;
-                        if (t1 >= a.hdisc && t1 < M - a.hdisc) outd[(size_t)((t1 - a.hdisc) >> LOGD) * nchan_total] = s1 * a.scale;
+                        if (t1 >= a.hdisc && t1 < M - a.hdisc) {
+                            const float f = s1 * a.scale;
+                            outd[(size_t)((t1 - a.hdisc) >> LOGD) * nchan_total] = f;
+                            mine[(2 * kk + 1) & 3] = f;
+                        }
                     }
                 }
+                // block sums (Alg. 1 l.104): the values go to the chirp warp of this quadrant, which adds them in
+                // fp64; it reads slot dd after the `empty` barrier of trial dd + 1, which this warp reaches later
+                if (SUMS)
+                    fsum[((size_t)((unsigned)(dd - d_begin) & (G::SUM_SLOTS - 1)) * G::NGRP + g) * NT + t] =
+                        make_float4(mine[0], mine[1], mine[2], mine[3]);
             };
 
 #pragma unroll 1
@@ -429,7 +489,9 @@ template <int M, int LOGD>
 static cudaError_t launch_ws_MD(FusedArgs fa, const double *h_dm, int nunits, cudaStream_t st, long long *launches)
 {
     using G = WS<M>;
-    cudaError_t e = cudaFuncSetAttribute(k_fused_ws<M, LOGD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem_bytes);
+    const bool sums = fa.segsum != nullptr;
+    cudaError_t e = sums ? cudaFuncSetAttribute(k_fused_ws<M, LOGD, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem_bytes)
+                         : cudaFuncSetAttribute(k_fused_ws<M, LOGD, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem_bytes);
     if (e != cudaSuccess) return e;
     const int ndm_total = fa.ndm;
     fa.nb_chunk = nunits / fa.nsub;
@@ -443,7 +505,8 @@ static cudaError_t launch_ws_MD(FusedArgs fa, const double *h_dm, int nunits, cu
         fa.dm_param0 = d0;
         fa.ndm = d0 + cnt;
         dim3 grid((unsigned)(npairs * fa.nchan), (unsigned)((cnt + fa.dm_tile - 1) / fa.dm_tile));
-        k_fused_ws<M, LOGD><<<grid, G::NTHREADS, G::smem_bytes, st>>>(fa, dmp);
+        if (sums) k_fused_ws<M, LOGD, true><<<grid, G::NTHREADS, G::smem_bytes, st>>>(fa, dmp);
+        else k_fused_ws<M, LOGD, false><<<grid, G::NTHREADS, G::smem_bytes, st>>>(fa, dmp);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
         ++*launches;

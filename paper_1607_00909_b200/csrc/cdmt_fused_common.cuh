@@ -49,6 +49,8 @@ struct FusedArgs {
     int unit0, nsub, nchan, nfft, hdisc, ndec, vdec, ndm, dm_tile, chirp_ref, accurate;
     int dm_first, dm_param0;  // DM range [dm_first, ndm) of this launch; dmp.dm[0] is trial dm_param0
     int nb_chunk;             // k_fused_ws: whole blocks in this chunk (units = nb_chunk * nsub)
+    double2 *segsum;          // block sums [ndm][nblock_total][nsub nchan] of (I, I^2) (Alg. 1 l.104), or null
+    int nblock_total;         // blocks of this execute (second dimension of segsum)
     double bw_mhz;
     float scale;
 };
@@ -104,6 +106,18 @@ __device__ __forceinline__ void lane_reduce_scatter(float *a, int lane)
             a[j] = keep + __shfl_xor_sync(0xffffffffu, send, 1 << S);
         }
         lane_reduce_scatter<LOGD, S + 1>(a, lane);
+    }
+}
+
+// Block sums of Alg. 1 l.104 inside a packed fused kernel: every thread adds the float32 values it has
+// just stored (sum and sum of squares, fp64), the warp reduces them by shuffles and lane 0 leaves the
+// warp's pair in shared memory; one thread adds the warps' pairs later (see the kernels).
+__device__ __forceinline__ void warp_sum_pair(double &a, double &q)
+{
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        a += __shfl_xor_sync(0xffffffffu, a, off);
+        q += __shfl_xor_sync(0xffffffffu, q, off);
     }
 }
 

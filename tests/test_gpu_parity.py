@@ -160,10 +160,10 @@ def test_fused_kernel_variants(cdmt, shape, ref):
         worst = check_filterbank(got, want)
         assert worst < TOL, (kern, worst)
     if 4 in kerns:
-        # kernel 4 pairs the blocks of a chunk: one block per chunk (second FFT group idle), a DM tile that
-        # does not divide ndm, and chunks of two blocks (ragged last chunk where nblock is odd)
-        for opts in ({cdmt.OPT_CHUNK_UNITS: nsub, cdmt.OPT_DM_TILE: 2}, {cdmt.OPT_CHUNK_UNITS: 2 * nsub}):
-            opts[cdmt.OPT_FUSED_KERNEL] = 4
+        # kernel 4 pairs the blocks of a chunk: chunks of three blocks (the third block's CTAs run with the
+        # second FFT group idle) with a DM tile that does not divide ndm, and chunks of two blocks (where
+        # nblock is odd the last chunk is a lone block, which goes to kernel 3)
+        for opts in ({cdmt.OPT_CHUNK_UNITS: 3 * nsub, cdmt.OPT_DM_TILE: 2}, {cdmt.OPT_CHUNK_UNITS: 2 * nsub}):
             got, _ = gpu_run(cdmt, cfg, x, ref, opts=opts)
             check_filterbank(got, want)
     # a DM tile that does not divide ndm, one unit per chunk
