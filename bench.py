@@ -437,38 +437,79 @@ def main():
             redig = {"error": str(e)}
 
     # ---- extra (not part of `value`): incoherent dedispersion of every coherent filterbank over fine DM
-    # offsets spanning the coherent DM step at PAPER.md:141's 0.002 pc/cm3 (semi-coherent search);
-    # FP32-add bound: one add per (coherent DM, fine trial, channel, output sample)
+    # offsets spanning the coherent DM step at PAPER.md:141's 0.002 pc/cm3 (semi-coherent search), streamed
+    # group by group: execute writes each block group behind the shift_range rows carried over from the
+    # previous one, so the stage also runs where the filterbanks are never resident at once (c5).
     incoh = None
-    if not args.no_incoherent and groups == 1:
+    if not args.no_incoherent:
         try:
             dm_step = float(cfg.dm[1] - cfg.dm[0]) if cfg.ndm > 1 else 1.0
             nhalf = int(round(0.5 * dm_step / args.fine_step))
             ddm = np.round(np.arange(-nhalf, nhalf + 1) * args.fine_step, 9)
             qi = cdmt.cdmt_incoherent_query(plan, ddm, nt)
-            d_ts = torch.empty((cfg.ndm, len(ddm), qi["nt_out"]), dtype=torch.float32, device=dev)
+            R, nout = qi["shift_range"], qi["nt_out"]
+            rows_g = nb_group * cfg.nvalid_dec
+            del out
+            torch.cuda.empty_cache()
+            win = torch.empty((cfg.ndm, R + rows_g, nch), dtype=torch.float32, device=dev)
+            out = win[:, R:]                               # where cdmt_execute writes a group
+            d_ts = torch.empty((cfg.ndm, len(ddm), nout), dtype=torch.float32, device=dev)
             d_iws = torch.empty(max(256, qi["workspace_bytes"]), dtype=torch.uint8, device=dev)
-            i0, i1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            esz = 2 if int8 else 8
+            wstride = win[0].numel()
+
+            def semicoherent_step(timers=None):
+                done = 0
+                for gi, b0 in enumerate(range(0, nb_total, nb_group)):
+                    nb = min(nb_group, nb_total - b0)
+                    ns = (nb - 1) * cfg.step + cfg.nfft
+                    cdmt.cdmt_execute(plan, d_in.data_ptr() + b0 * cfg.step * esz, ns, cfg.nsamp, out.data_ptr(),
+                                      wstride, ws, ws.numel(), stream)
+                    n = nb * cfg.nvalid_dec
+                    nt_in = n if gi == 0 else R + n
+                    src = out.data_ptr() if gi == 0 else win.data_ptr()
+                    if timers is not None:
+                        ev = torch.cuda.Event(enable_timing=True); ev.record(stream); timers.append(ev)
+                    cdmt.cdmt_incoherent_dedisperse(plan, src, wstride, nt_in, ddm, d_ts.data_ptr() + 4 * done,
+                                                    d_ts[0].numel(), nout, d_iws, d_iws.numel(), stream)
+                    if b0 + nb < nb_total:
+                        cdmt.cdmt_incoherent_carry(plan, win, wstride, R + n, R, stream)
+                    if timers is not None:
+                        ev = torch.cuda.Event(enable_timing=True); ev.record(stream); timers.append(ev)
+                    done += nt_in - R
+                return done
+
+            assert semicoherent_step() == nout             # warm-up
             reps = 2
-            for i in range(reps + 1):
-                if i == 1:
-                    i0.record(stream)
-                cdmt.cdmt_incoherent_dedisperse(plan, out, out[0].numel(), nt, ddm, d_ts, d_ts[0].numel(),
-                                                qi["nt_out"], d_iws, d_iws.numel(), stream)
+            i0, i1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            timers = []
+            i0.record(stream)
+            for _ in range(reps):
+                semicoherent_step(timers)
             i1.record(stream)
             torch.cuda.synchronize()
-            ims = i0.elapsed_time(i1) / reps
-            adds = float(cfg.ndm) * len(ddm) * nch * qi["nt_out"]
+            step_ms = i0.elapsed_time(i1) / reps
+            ims = sum(timers[2 * k].elapsed_time(timers[2 * k + 1]) for k in range(len(timers) // 2)) / reps
+            adds_def, adds_done = cdmt.cdmt_incoherent_work(plan, ddm, nt)
             peak_add = 148 * 128 * 1.965e9 / 1e12
-            incoh = {"ms_per_call": ims, "fine_trials": len(ddm), "fine_step": args.fine_step,
-                     "trial_groups": qi["ngroups"], "shift_range": qi["shift_range"], "adds": adds,
-                     "achieved_tadd_s": adds / ims / 1e9, "peak_tadd_s": peak_add,
-                     "frac": adds / ims / 1e9 / peak_add, "bound": "alu",
+            # shared-memory bound: every addition the kernel performs reads at most one 4-byte word; the
+            # register window makes it (8 + spread) words per 8 (1 + spread) additions
+            incoh = {"ms_per_step": ims, "groups": groups, "fine_trials": len(ddm), "fine_step": args.fine_step,
+                     "trial_groups": qi["ngroups"], "shift_range": R,
+                     "adds_definition": adds_def, "adds_performed": adds_done,
+                     "speedup_over_definition": adds_def / adds_done,
+                     "bound": "alu", "achieved_tadd_s": adds_done / ims / 1e9, "peak_tadd_s": peak_add,
+                     "frac": adds_done / ims / 1e9 / peak_add,
+                     "definition_tadd_s": adds_def / ims / 1e9,
                      "peak_source": "derived: 148 SM x 128 FP32 lanes x 1.965 GHz (one FADD per lane and clock)",
-                     "out_bytes": int(d_ts.numel() * 4),
-                     "note": "cdmt_incoherent_dedisperse on the step's filterbanks; not included in value; `adds` is "
-                             "the count of the brute-force definition (the kernel shares sums between trials)"}
-            del d_ts, d_iws
+                     "out_bytes": int(d_ts.numel() * 4), "semicoherent_step_ms": step_ms,
+                     "note": "cdmt_incoherent_dedisperse (+ cdmt_incoherent_carry) on every block group of the step, "
+                             "streamed through a window of shift_range + group rows; not included in value; `frac` "
+                             "counts the additions the kernel performs (runs of channels that share their shifts are "
+                             "summed once per distinct shift), `definition_tadd_s` those of the brute-force "
+                             "definition; semicoherent_step_ms = execute + incoherent for the whole observation"}
+            del d_ts, d_iws, win
+            out = None
         except Exception as e:
             incoh = {"error": str(e)}
 
@@ -477,7 +518,7 @@ def main():
     e2e = None
     e2e_u8 = None
     if want_e2e:
-        del out
+        out = None
         torch.cuda.empty_cache()
         ksteps = max(1, min(args.steps, 3))
 

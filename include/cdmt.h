@@ -142,10 +142,11 @@ int cdmt_execute(cdmt_plan *plan, const void *d_in, long long nsamp, long long i
  *   d_segsum   DEVICE fp64 [ndm][nblock][nsub*nchan][2] = (sum I, sum I^2) over the Vd float32
  *              samples that block b gave channel j (output order) at trial d; dense;
  *              cdmt_redigitize_workspace_bytes() bytes, 16-byte aligned.
- * The packed fused kernels take the sums from the values they are about to store (each CTA owns
- * exactly one such segment), so the filterbank is not read back for them; for shapes that run on the
- * general kernels the sums come from a separate pass over d_out.  Feed them to
- * cdmt_redigitize_sums.  Same errors as cdmt_execute.
+ * The warp-specialised fused kernel (nfft/nchan = 4096, ndec 8, 16 or 32) takes the sums from the
+ * values it is about to store -- each CTA owns whole segments, and its chirp warps have the time --
+ * so the filterbank is not read back for them; for every other shape the sums come from a separate
+ * pass over d_out (on this hardware cheaper than fp64 sums inside an ALU-bound kernel).  Feed them
+ * to cdmt_redigitize_sums.  Same errors as cdmt_execute.
  */
 int cdmt_execute_sums(cdmt_plan *plan, const void *d_in, long long nsamp, long long in_stride_pol,
                       float *d_out, long long out_stride_dm, double *d_segsum, void *d_workspace,
@@ -258,12 +259,26 @@ int cdmt_redigitize_sums(cdmt_plan *plan, const float *d_fb, long long fb_stride
  * of trial groups the kernel works in (<= 8 trials each; fewer where the shifts of consecutive
  * trials differ by more than the kernel's register window allows).
  * cdmt_incoherent_shifts: copies the shift table [nfine][nsub*nchan] to HOST memory.
- * Sums are accumulated in float32 in channel order.  The plan caches the shift and group tables of the
- * last ddm list it was given (these three calls therefore take a non-const plan and, like every other
- * call, must not run concurrently on one plan); cdmt_incoherent_dedisperse uploads them with
- * cudaMemcpyAsync from pageable host memory on `cuda_stream` and queues one kernel.
+ * Sums are accumulated in float32; the terms of a trial are those of the definition above, added in
+ * another order (channels that share their shifts over a group of trials are summed once), so results
+ * are exact on integer-valued data and equal to the definition to float32 rounding otherwise.  The plan
+ * caches the shift and group tables of the last ddm list it was given (these calls therefore take a
+ * non-const plan and, like every other call, must not run concurrently on one plan) and, from the first
+ * cdmt_incoherent_dedisperse on, a page-locked copy of them: the call queues two asynchronous copies
+ * from that memory and one kernel on `cuda_stream`, nothing else (capturable into a CUDA graph).
+ * Limits (CDMT_ERR_SIZE from all three calls): shift_range <= about 14000 samples (four channels of
+ * 256 + shift_range samples must fit shared memory), at most 16 x 65535 trial groups.
+ *
+ * Streaming over block groups (40 000 trials over a 20-minute observation are never
+ * resident): keep per DM plane a window of shift_range + nt_group rows; let cdmt_execute write each
+ * group's rows behind the first shift_range rows (pass d_out + shift_range * nsub*nchan and the
+ * window's plane stride); dedisperse the window (the first group without the empty head: nt_in =
+ * nt_group, giving nt_group - shift_range samples; every later one with nt_in = shift_range +
+ * nt_group, giving nt_group samples that continue the series); then cdmt_incoherent_carry moves the
+ * last shift_range rows of every plane to its front (needs nt_in >= 2 shift_range).  The
+ * concatenated outputs are bit for bit those of one call on the whole span.
  * Errors: CDMT_ERR_ARG (null / misaligned pointer, non-finite or non-ascending ddm), CDMT_ERR_SIZE
- * (nt_in <= shift_range, short strides), CDMT_ERR_WORKSPACE, CDMT_ERR_ALLOC, CDMT_ERR_CUDA.
+ * (nt_in <= shift_range, short strides, limits above), CDMT_ERR_WORKSPACE, CDMT_ERR_ALLOC, CDMT_ERR_CUDA.
  */
 int cdmt_incoherent_query(cdmt_plan *plan, int nfine, const double *ddm, long long nt_in,
                           int *shift_min, int *shift_range, long long *nt_out, int *ngroups,
@@ -273,6 +288,14 @@ int cdmt_incoherent_dedisperse(cdmt_plan *plan, const float *d_fb, long long fb_
                                long long nt_in, int nfine, const double *ddm, float *d_ts,
                                long long ts_stride_dm, long long ts_pitch, void *d_workspace,
                                size_t workspace_bytes, void *cuda_stream);
+int cdmt_incoherent_carry(cdmt_plan *plan, float *d_fb, long long fb_stride_dm, long long nt_in,
+                          int shift_range, void *cuda_stream);
+/* Additions per call of cdmt_incoherent_dedisperse over all DM planes (host arithmetic): those of the
+ * brute-force definition (one per plane, trial, channel and output sample) and those the kernel
+ * performs (one per plane, trial group, channel, DISTINCT shift and sample, plus the hand-over of the
+ * run sums to the trials). */
+int cdmt_incoherent_work(cdmt_plan *plan, int nfine, const double *ddm, long long nt_in,
+                         double *adds_definition, double *adds_performed);
 
 /* Eq. 2: dispersion sweep across [fcen - bw/2, fcen + bw/2] in seconds. */
 double cdmt_sweep_seconds(double fcen_mhz, double bw_mhz, double dm);

@@ -30,7 +30,7 @@ EXPORTS = [
     "cdmt_execute", "cdmt_execute_sums", "cdmt_execute_host", "cdmt_execute_host_async", "cdmt_host_layout",
     "cdmt_host_scratch_bytes", "cdmt_host_traffic_bytes", "cdmt_unpack",
     "cdmt_forward_spectrum", "cdmt_redigitize", "cdmt_redigitize_sums", "cdmt_redigitize_workspace_bytes",
-    "cdmt_incoherent_query", "cdmt_incoherent_shifts", "cdmt_incoherent_dedisperse",
+    "cdmt_incoherent_query", "cdmt_incoherent_shifts", "cdmt_incoherent_dedisperse", "cdmt_incoherent_carry", "cdmt_incoherent_work",
     "cdmt_sweep_seconds", "cdmt_min_overlap", "cdmt_suggest_sizes",
     "cdmt_measure_fp32_peak", "cdmt_last_launch_count", "cdmt_profile_read", "cdmt_strerror",
     "cdmt_version",
@@ -67,6 +67,8 @@ _lib.cdmt_incoherent_query.argtypes = [_vp, _i, C.POINTER(_d), _ll, C.POINTER(_i
                                        C.POINTER(_i), C.POINTER(_sz)]
 _lib.cdmt_incoherent_shifts.argtypes = [_vp, _i, C.POINTER(_d), _vp]
 _lib.cdmt_incoherent_dedisperse.argtypes = [_vp, _vp, _ll, _ll, _i, C.POINTER(_d), _vp, _ll, _ll, _vp, _sz, _vp]
+_lib.cdmt_incoherent_carry.argtypes = [_vp, _vp, _ll, _ll, _i, _vp]
+_lib.cdmt_incoherent_work.argtypes = [_vp, _i, C.POINTER(_d), _ll, C.POINTER(_d), C.POINTER(_d)]
 _lib.cdmt_sweep_seconds.argtypes = [_d, _d, _d]
 _lib.cdmt_sweep_seconds.restype = _d
 _lib.cdmt_suggest_sizes.argtypes = [_i, C.POINTER(_d), _d, _i, _i, _d, _i, _d, C.POINTER(_i), C.POINTER(_i)]
@@ -284,6 +286,18 @@ def cdmt_incoherent_dedisperse(plan: Plan, d_fb, fb_stride_dm: int, nt_in: int, 
                                          _ptr(d_ts), int(ts_stride_dm), int(ts_pitch), _ptr(d_workspace),
                                          int(workspace_bytes), _stream(stream))
     _check(st, "cdmt_incoherent_dedisperse")
+
+
+def cdmt_incoherent_carry(plan: Plan, d_fb, fb_stride_dm: int, nt_in: int, shift_range: int, stream=None):
+    _check(_lib.cdmt_incoherent_carry(plan.handle, _ptr(d_fb), int(fb_stride_dm), int(nt_in), int(shift_range),
+                                      _stream(stream)), "cdmt_incoherent_carry")
+
+
+def cdmt_incoherent_work(plan: Plan, ddm, nt_in: int):
+    a, pa = _ddm(ddm)
+    x, y = _d(), _d()
+    _check(_lib.cdmt_incoherent_work(plan.handle, a.size, pa, int(nt_in), C.byref(x), C.byref(y)), "cdmt_incoherent_work")
+    return x.value, y.value
 
 
 def cdmt_min_overlap(plan: Plan) -> int:

@@ -164,6 +164,7 @@ extern "C" int cdmt_plan_destroy(cdmt_plan *plan)
 {
     if (!plan) return CDMT_ERR_ARG;
     for (cudaEvent_t e : plan->ev_pool) cudaEventDestroy(e);
+    incoherent_release(&plan->ic);
     if (plan->host_ready) {
         cudaStreamDestroy(plan->s_in);
         cudaStreamDestroy(plan->s_out);
@@ -750,6 +751,8 @@ static int plan_incoherent(cdmt_plan *plan, int nfine, const double *ddm)
     try {
         plan->ic_ddm.clear();
         if (!incoherent_plan(plan->g, plan->fcen.data(), nfine, ddm, &plan->ic)) return CDMT_ERR_ARG;
+        // shift range beyond the shared-memory tile, or more trial groups than a grid dimension holds
+        if (!incoherent_config(plan->ic, nullptr, nullptr, nullptr)) return CDMT_ERR_SIZE;
         plan->ic_ddm.assign(ddm, ddm + nfine);
     } catch (...) {
         plan->ic_ddm.clear();
@@ -796,11 +799,44 @@ extern "C" int cdmt_incoherent_dedisperse(cdmt_plan *plan, const float *d_fb, lo
     const long long nt_out = nt_in - plan->ic.range;
     if (nt_in < 1 || nt_in > (1LL << 30) || nt_out < 1) return CDMT_ERR_SIZE;
     if (fb_stride_dm < nt_in * nch || ts_pitch < nt_out || ts_stride_dm < (long long)nfine * ts_pitch) return CDMT_ERR_SIZE;
-    if (g.ndm > 65535 || plan->ic.groups.size() / 4 > 65535) return CDMT_ERR_SIZE;
+    if (g.ndm > 65535) return CDMT_ERR_SIZE;
     if (workspace_bytes < incoherent_workspace_bytes(plan->ic)) return CDMT_ERR_WORKSPACE;
     plan->last_launches = 0;
     return check_cuda(launch_incoherent(g, plan->ic, d_fb, fb_stride_dm, nt_in, d_ts, ts_stride_dm, ts_pitch,
                                         d_workspace, static_cast<cudaStream_t>(cuda_stream), &plan->last_launches));
+}
+
+extern "C" int cdmt_incoherent_work(cdmt_plan *plan, int nfine, const double *ddm, long long nt_in,
+                                    double *adds_definition, double *adds_performed)
+{
+    int rc = plan_incoherent(plan, nfine, ddm);
+    if (rc) return rc;
+    const IncoherentTables &T = plan->ic;
+    const double nt_out = (double)(nt_in - T.range);
+    if (nt_out < 1.0) return CDMT_ERR_SIZE;
+    double steps = 0.0, run_ends = 0.0;
+    for (const uint2 &e : T.entries) {
+        steps += 1.0 + (double)((e.x >> 24) & 7u);
+        if (e.x & (1u << 28)) run_ends += 1.0;
+    }
+    if (adds_definition) *adds_definition = (double)plan->g.ndm * nfine * T.nch * nt_out;
+    if (adds_performed) *adds_performed = (double)plan->g.ndm * nt_out * (steps + 8.0 * run_ends);
+    return CDMT_OK;
+}
+
+// Streaming the incoherent stage over block groups (the filterbanks of a 20-minute
+// observation are never resident at once): the last `shift_range` rows of every plane become the first.
+extern "C" int cdmt_incoherent_carry(cdmt_plan *plan, float *d_fb, long long fb_stride_dm, long long nt_in,
+                                     int shift_range, void *cuda_stream)
+{
+    if (!plan || !d_fb || (reinterpret_cast<uintptr_t>(d_fb) & 3) != 0) return CDMT_ERR_ARG;
+    const Geometry &g = plan->g;
+    const long long nch = (long long)g.nsub * g.nchan;
+    if (shift_range < 0 || nt_in < 2LL * shift_range || fb_stride_dm < nt_in * nch) return CDMT_ERR_SIZE;
+    if (g.ndm > 65535) return CDMT_ERR_SIZE;
+    plan->last_launches = 0;
+    return check_cuda(launch_carry_rows(d_fb, fb_stride_dm, nt_in, shift_range, (int)nch, g.ndm,
+                                        static_cast<cudaStream_t>(cuda_stream), &plan->last_launches));
 }
 
 // n_d n_c >= r t_d for the lowest-frequency channel (or subband) at the largest |DM|.

@@ -438,15 +438,16 @@ cudaError_t launch_fused(const Geometry &g, const Workspace &ws, const float2 *s
     if (force_generic == 2 && !fast_ok) return cudaErrorInvalidValue;
     // automatic choice: x2 (measured fastest on all five configs: c3 21.8 ms per launch against 22.2 for sp),
     // then sp (covers ndec < 8)
-    // the two packed half-transform kernels take the block sums of l.104 themselves
-    if ((ws_ok && (force_generic == 0 || force_generic == 4)) || (x2_ok && (force_generic == 0 || force_generic == 3))) {
-        fa.segsum = reinterpret_cast<double2 *>(d_segsum);
-        if (d_segsum && sums_done) *sums_done = true;
-    }
     // automatic choice: ws needs at least one full pair of blocks (a lone block would leave the second FFT
     // group of every CTA idle: x2 is faster there)
-    if (ws_ok && ((force_generic == 0 && nunits >= 2 * g.nsub) || force_generic == 4))
+    if (ws_ok && ((force_generic == 0 && nunits >= 2 * g.nsub) || force_generic == 4)) {
+        // the warp-specialised kernel takes the block sums of l.104 itself (its chirp warps have the time);
+        // in k_fused_x2 the same fp64 sums cost 7 % of the kernel (c5: 139 ms against 23 ms for the separate
+        // pass over the filterbank), so every other kernel leaves them to launch_block_sums
+        fa.segsum = reinterpret_cast<double2 *>(d_segsum);
+        if (d_segsum && sums_done) *sums_done = true;
         return launch_fused_ws(M, logd, fa, h_dm, nunits, st, launches);
+    }
     if (x2_ok && (force_generic == 0 || force_generic == 3)) return launch_fused_x2(M, logd, fa, h_dm, nunits, st, launches);
     if (sp_ok && (force_generic == 0 || force_generic == 5)) return launch_fused_sp(M, logd, fa, h_dm, nunits, st, launches);
     const bool fast = fast_ok && force_generic != 1;

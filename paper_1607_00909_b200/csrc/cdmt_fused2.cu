@@ -48,8 +48,7 @@ struct X2 {
     static constexpr int TCOLS = COLS_SLOT * ((NWARP + 3) / 4);
     static constexpr int COL_X = 0, COL_TW1 = 128, COL_TW2 = 160, COL_TWF = 192;
     static constexpr size_t smem_bytes =
-        sizeof(float4) * 2 * EX + sizeof(float2) * NWARP * INTEG + sizeof(double) * 12 * NT + 32 +
-        sizeof(double2) * 2 * NWARP;
+        sizeof(float4) * 2 * EX + sizeof(float2) * NWARP * INTEG + sizeof(double) * 12 * NT + 32;
     static constexpr int CTAS_PER_SM = 512 / TCOLS;  // bounded by tensor memory
 };
 
@@ -99,7 +98,7 @@ __device__ __forceinline__ void x2_chirp(const double *coef, int tid, double dm,
     }
 }
 
-template <int M, int LOGD, bool SUMS>
+template <int M, int LOGD>
 __global__ void __launch_bounds__(M / 32, X2<M>::CTAS_PER_SM)
 k_fused_x2(const FusedArgs a, const __grid_constant__ DmParams dmp)
 {
@@ -115,7 +114,6 @@ k_fused_x2(const FusedArgs a, const __grid_constant__ DmParams dmp)
     uint64_t *bar = reinterpret_cast<uint64_t *>(coef + 12 * NT);  // pass-2 loads done (buffers free)
     uint64_t *barA = bar + 1;                                      // pass-1 stores done
     uint32_t *tslot = reinterpret_cast<uint32_t *>(barA + 1);
-    double2 *wsum = reinterpret_cast<double2 *>(tslot + 4);  // [2][NWARP]: the warps' (sum I, sum I^2) of a trial
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int c = blockIdx.x % a.nchan;
@@ -260,16 +258,6 @@ k_fused_x2(const FusedArgs a, const __grid_constant__ DmParams dmp)
         mbar_arrive(barA);
         if (d + 1 < d_end) x2_chirp<NT>(coef, tid, dmp.dm[d + 1 - a.dm_param0], Hr, Hi);
         mbar_wait(barA, par);
-        if (SUMS && tid == 0 && d != d_begin) {
-            // every warp left its pair of trial d-1 before it arrived at this barrier
-            double a1 = 0.0, a2 = 0.0;
-#pragma unroll
-            for (int w = 0; w < G::NWARP; ++w) {
-                a1 += wsum[(par ^ 1u) * G::NWARP + w].x;
-                a2 += wsum[(par ^ 1u) * G::NWARP + w].y;
-            }
-            a.segsum[((size_t)(d - 1) * a.nblock_total + b) * nchan_total + ochan] = make_double2(a1, a2);
-        }
         // ---- pass 2 along j2, radix-2 combine, detection, polarisation sum
         P2 pw[16];  // (|y[t']|^2, |y[t' + L]|^2) summed over polarisations, order k = u R2 + t2
         {
@@ -324,7 +312,6 @@ k_fused_x2(const FusedArgs a, const __grid_constant__ DmParams dmp)
         float *outd = out0 + (size_t)d * (size_t)a.out_stride_dm;
         const int i = lane & (DG - 1), g0 = lane - i;
         const int tgrp = (D > 16) ? (tid & ~31) : (tid - i);  // first sample of the group, before + NT n
-        double sum1 = 0.0, sum2 = 0.0;
 #pragma unroll
         for (int kk = 0; kk < 16 / DG; ++kk) {
             const int n = i + DG * kk;
@@ -343,36 +330,14 @@ k_fused_x2(const FusedArgs a, const __grid_constant__ DmParams dmp)
             }
             const int t0 = tgrp + NT * n;
             if (D <= 16 || lane < 16) {
-                if (t0 >= a.hdisc && t0 < M - a.hdisc) {
-                    const float f = s0 * a.scale;
-                    outd[(size_t)((t0 - a.hdisc) >> LOGD) * nchan_total] = f;
-                    if (SUMS) { sum1 += (double)f; sum2 = fma((double)f, (double)f, sum2); }
-                }
+                if (t0 >= a.hdisc && t0 < M - a.hdisc) outd[(size_t)((t0 - a.hdisc) >> LOGD) * nchan_total] = s0 * a.scale;
                 const int t1 = t0 + L;
-                if (t1 >= a.hdisc && t1 < M - a.hdisc) {
-                    const float f = s1 * a.scale;
-                    outd[(size_t)((t1 - a.hdisc) >> LOGD) * nchan_total] = f;
-                    if (SUMS) { sum1 += (double)f; sum2 = fma((double)f, (double)f, sum2); }
-                }
+                if (t1 >= a.hdisc && t1 < M - a.hdisc) outd[(size_t)((t1 - a.hdisc) >> LOGD) * nchan_total] = s1 * a.scale;
             }
-        }
-        if (SUMS) {
-            warp_sum_pair(sum1, sum2);
-            if (lane == 0) wsum[par * G::NWARP + warp] = make_double2(sum1, sum2);
         }
     }
     tmem_fence_before_sync();
     __syncthreads();
-    if (SUMS && tid == 0 && d_begin < d_end) {
-        const unsigned par = (unsigned)(d_end - 1 - d_begin) & 1u;
-        double a1 = 0.0, a2 = 0.0;
-#pragma unroll
-        for (int w = 0; w < G::NWARP; ++w) {
-            a1 += wsum[par * G::NWARP + w].x;
-            a2 += wsum[par * G::NWARP + w].y;
-        }
-        a.segsum[((size_t)(d_end - 1) * a.nblock_total + b) * nchan_total + ochan] = make_double2(a1, a2);
-    }
     if (warp == 0) tmem_dealloc<G::TCOLS>(tbase);
 }
 
@@ -387,9 +352,7 @@ static cudaError_t launch_x2_MD(FusedArgs fa, const double *h_dm, int nunits, cu
     size_t smem = G::smem_bytes;
     const size_t floor_bytes = (size_t)(233472 / (G::CTAS_PER_SM + 1)) - 1024 + 16;
     if (smem < floor_bytes) smem = floor_bytes;
-    const bool sums = fa.segsum != nullptr;
-    cudaError_t e = sums ? cudaFuncSetAttribute(k_fused_x2<M, LOGD, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
-                         : cudaFuncSetAttribute(k_fused_x2<M, LOGD, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(k_fused_x2<M, LOGD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const int ndm_total = fa.ndm;
     for (int d0 = 0; d0 < ndm_total; d0 += DM_PARAM_MAX) {
@@ -401,8 +364,7 @@ static cudaError_t launch_x2_MD(FusedArgs fa, const double *h_dm, int nunits, cu
         fa.dm_param0 = d0;
         fa.ndm = d0 + cnt;
         dim3 grid((unsigned)(nunits * fa.nchan), (unsigned)((cnt + fa.dm_tile - 1) / fa.dm_tile));
-        if (sums) k_fused_x2<M, LOGD, true><<<grid, M / 32, smem, st>>>(fa, dmp);
-        else k_fused_x2<M, LOGD, false><<<grid, M / 32, smem, st>>>(fa, dmp);
+        k_fused_x2<M, LOGD><<<grid, M / 32, smem, st>>>(fa, dmp);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
         ++*launches;

@@ -28,6 +28,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdint>
+#include <cstring>
 
 #include "cdmt_internal.h"
 
@@ -45,6 +46,7 @@ bool incoherent_plan(const Geometry &g, const double *h_fcen, int nfine, const d
     for (int k = 1; k < nfine; ++k)
         if (!(ddm[k] > ddm[k - 1])) return false;
     const int nch = g.nsub * g.nchan;
+    incoherent_release(T);   // page-locked copy of the previous tables
     T->nfine = nfine;
     T->nch = nch;
     // channel centres in the order of the filterbank: descending frequency
@@ -66,7 +68,7 @@ bool incoherent_plan(const Geometry &g, const double *h_fcen, int nfine, const d
         }
     T->smin = smin;
     T->range = smax - smin;
-    // groups of up to 16 consecutive trials whose shifts grow by at most 3 samples per trial and 4 in all
+    // groups of up to 8 consecutive trials whose shifts grow by at most 3 samples per trial and 4 in all
     T->groups.clear();
     T->entries.clear();
     int k0 = 0;
@@ -310,38 +312,84 @@ __global__ void __launch_bounds__(32 * IC_WARPS, 1) k_incoherent(const IcArgs a)
     }
 }
 
-// ---------------------------------------------------------------------------------------- launch
-cudaError_t launch_incoherent(const Geometry &g, const IncoherentTables &T, const float *d_fb, long long fb_stride_dm,
-                              long long nt_in, float *d_ts, long long ts_stride_dm, long long ts_pitch,
-                              void *d_workspace, cudaStream_t st, long long *launches)
+// the last `nrows` rows of every DM plane move to its front (cdmt_incoherent_carry)
+__global__ void __launch_bounds__(256) k_carry_rows(float *fb, long long fb_stride_dm, long long src_off, long long n)
 {
-    const int nch = T.nch, ngroups = (int)T.groups.size();
-    const long long nt_out = nt_in - T.range;
-    char *ws = reinterpret_cast<char *>(d_workspace);
-    uint2 *d_entries = reinterpret_cast<uint2 *>(ws);
-    int2 *d_groups = reinterpret_cast<int2 *>(ws + ic_align(T.entries.size() * sizeof(uint2)));
-    cudaError_t e = cudaMemcpyAsync(d_entries, T.entries.data(), T.entries.size() * sizeof(uint2), cudaMemcpyHostToDevice, st);
-    if (e != cudaSuccess) return e;
-    e = cudaMemcpyAsync(d_groups, T.groups.data(), T.groups.size() * sizeof(int2), cudaMemcpyHostToDevice, st);
-    if (e != cudaSuccess) return e;
+    float *p = fb + (size_t)blockIdx.y * (size_t)fb_stride_dm;
+    for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < n; i += (long long)gridDim.x * 256) p[i] = p[src_off + i];
+}
 
-    IcArgs a;
-    a.fb = d_fb; a.fb_stride_dm = fb_stride_dm; a.ts = d_ts; a.ts_stride_dm = ts_stride_dm; a.ts_pitch = ts_pitch;
-    a.entries = d_entries; a.groups = d_groups;
-    a.nt_in = (int)nt_in; a.nt_out = (int)nt_out; a.nch = nch; a.ngroups = ngroups;
-    a.tw = ((T.range + IC_TILE + 30) & ~31) + 1;  // >= range + 256 and = 1 mod 32
-    a.vec_in = (nch % 4 == 0 && fb_stride_dm % 4 == 0 && (reinterpret_cast<uintptr_t>(d_fb) & 15) == 0) ? 1 : 0;
+cudaError_t launch_carry_rows(float *d_fb, long long fb_stride_dm, long long nt_in, int nrows, int nch, int ndm,
+                              cudaStream_t st, long long *launches)
+{
+    const long long n = (long long)nrows * nch;
+    if (n == 0) return cudaSuccess;
+    dim3 grid((unsigned)((n + 256 * 8 - 1) / (256 * 8) > 4096 ? 4096 : (n + 256 * 8 - 1) / (256 * 8)), (unsigned)ndm);
+    k_carry_rows<<<grid, 256, 0, st>>>(d_fb, fb_stride_dm, (nt_in - nrows) * (long long)nch, n);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) ++*launches;
+    return e;
+}
+
+// ---------------------------------------------------------------------------------------- launch
+// Tile geometry for a shift range: the row length (>= range + 256 and = 1 mod 32) and the channels per
+// chunk that fit shared memory; false if even four channels do not fit (range > ~14000) or there are more
+// trial groups than a grid dimension holds.
+bool incoherent_config(const IncoherentTables &T, int *cc_out, int *tw_out, size_t *smem_out)
+{
+    const int tw = ((T.range + IC_TILE + 30) & ~31) + 1;
+    auto smem_for = [&](int cc) { return sizeof(float) * (((size_t)cc * tw + 3) & ~(size_t)3) + sizeof(uint2) * IC_WARPS * cc; };
     // channels per chunk: the largest of 32, 16, 8, 4 whose tile lets two CTAs share an SM, else whatever fits
-    auto smem_for = [&](int cc) { return sizeof(float) * (((size_t)cc * a.tw + 3) & ~(size_t)3) + sizeof(uint2) * IC_WARPS * cc; };
     int cc = 0;
     for (int c : {32, 16, 8, 4})
         if (smem_for(c) <= 72 * 1024) { cc = c; break; }
     if (!cc)
         for (int c : {32, 16, 8, 4})
             if (smem_for(c) <= 227 * 1024) { cc = c; break; }
-    if (!cc) return cudaErrorInvalidValue;
-    a.cc = cc;
-    const size_t smem = smem_for(cc);
+    if (!cc) return false;
+    if ((T.groups.size() + IC_WARPS - 1) / IC_WARPS > 65535) return false;   // grid.y
+    if (cc_out) *cc_out = cc;
+    if (tw_out) *tw_out = tw;
+    if (smem_out) *smem_out = smem_for(cc);
+    return true;
+}
+
+void incoherent_release(IncoherentTables *T)
+{
+    if (T->pinned) cudaFreeHost(T->pinned);
+    T->pinned = nullptr;
+}
+
+cudaError_t launch_incoherent(const Geometry &g, IncoherentTables &T, const float *d_fb, long long fb_stride_dm,
+                              long long nt_in, float *d_ts, long long ts_stride_dm, long long ts_pitch,
+                              void *d_workspace, cudaStream_t st, long long *launches)
+{
+    const int nch = T.nch, ngroups = (int)T.groups.size();
+    const long long nt_out = nt_in - T.range;
+    char *ws = reinterpret_cast<char *>(d_workspace);
+    const size_t nb_e = T.entries.size() * sizeof(uint2), nb_g = T.groups.size() * sizeof(int2);
+    uint2 *d_entries = reinterpret_cast<uint2 *>(ws);
+    int2 *d_groups = reinterpret_cast<int2 *>(ws + ic_align(nb_e));
+    // the tables travel from page-locked memory the plan keeps for them: a plain asynchronous copy on the
+    // caller's stream, also inside a stream capture
+    if (!T.pinned) {
+        cudaError_t e = cudaMallocHost(&T.pinned, ic_align(nb_e) + nb_g);
+        if (e != cudaSuccess) return e;
+        memcpy(T.pinned, T.entries.data(), nb_e);
+        memcpy(static_cast<char *>(T.pinned) + ic_align(nb_e), T.groups.data(), nb_g);
+    }
+    cudaError_t e = cudaMemcpyAsync(d_entries, T.pinned, nb_e, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return e;
+    e = cudaMemcpyAsync(d_groups, static_cast<char *>(T.pinned) + ic_align(nb_e), nb_g, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return e;
+
+    IcArgs a;
+    a.fb = d_fb; a.fb_stride_dm = fb_stride_dm; a.ts = d_ts; a.ts_stride_dm = ts_stride_dm; a.ts_pitch = ts_pitch;
+    a.entries = d_entries; a.groups = d_groups;
+    a.nt_in = (int)nt_in; a.nt_out = (int)nt_out; a.nch = nch; a.ngroups = ngroups;
+    size_t smem = 0;
+    if (!incoherent_config(T, &a.cc, &a.tw, &smem)) return cudaErrorInvalidValue;
+    a.vec_in = (nch % 4 == 0 && fb_stride_dm % 4 == 0 && (reinterpret_cast<uintptr_t>(d_fb) & 15) == 0) ? 1 : 0;
     e = cudaFuncSetAttribute(k_incoherent, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     dim3 grid((unsigned)((nt_out + IC_TILE - 1) / IC_TILE), (unsigned)((ngroups + IC_WARPS - 1) / IC_WARPS), (unsigned)g.ndm);

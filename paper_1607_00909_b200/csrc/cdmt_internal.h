@@ -71,14 +71,20 @@ struct IncoherentTables {            // host side, owned by the plan (must outli
     int smin = 0, range = 0;         // extremes of the shift table: range = smax - smin
     std::vector<int> shifts;         // [nfine][nch] samples, channel order of the filterbank (descending)
     std::vector<uint2> entries;      // [ngroups][nch]: x = first trial's shift - smin, y = 2-bit increments
-    std::vector<int2> groups;        // [ngroups]: (first trial, number of trials <= 16)
+    std::vector<int2> groups;        // [ngroups]: (first trial, number of trials <= 8)
+    void *pinned = nullptr;          // page-locked copy of entries + groups (made by the first dedisperse)
 };
 // Fills the tables; returns false if ddm is not ascending.
 bool incoherent_plan(const Geometry &g, const double *h_fcen, int nfine, const double *ddm, IncoherentTables *T);
 size_t incoherent_workspace_bytes(const IncoherentTables &T);
-cudaError_t launch_incoherent(const Geometry &g, const IncoherentTables &T, const float *d_fb, long long fb_stride_dm,
+// false if the shift range or the number of trial groups is beyond what the kernel can be launched with
+bool incoherent_config(const IncoherentTables &T, int *cc, int *tw, size_t *smem);
+void incoherent_release(IncoherentTables *T);
+cudaError_t launch_incoherent(const Geometry &g, IncoherentTables &T, const float *d_fb, long long fb_stride_dm,
                               long long nt_in, float *d_ts, long long ts_stride_dm, long long ts_pitch,
                               void *d_workspace, cudaStream_t st, long long *launches);
+cudaError_t launch_carry_rows(float *d_fb, long long fb_stride_dm, long long nt_in, int nrows, int nch, int ndm,
+                              cudaStream_t st, long long *launches);
 
 bool forward_len_supported(int L);
 bool fused_len_supported(int M);

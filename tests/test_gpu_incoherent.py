@@ -132,6 +132,48 @@ def test_incoherent_after_execute_end_to_end(cdmt):
         assert np.abs(got - ref["ts"]).max() <= 1e-3 * rms
 
 
+def test_incoherent_streams_over_block_groups_bit_exact(cdmt):
+    """the filterbanks of a long observation are never resident at once.  execute ->
+    incoherent runs group by group on a window of shift_range + nt_group rows (cdmt_incoherent_carry moves
+    the halo); on integer data the concatenated series equal ONE whole-span oracle call bit for bit."""
+    nsub, nchan, ndec, ndm = 12, 8, 2, 3
+    plan, p = make_plan(cdmt, nsub, nchan, ndec, ndm)
+    nch = nsub * nchan
+    ddm = np.round(np.arange(-0.25, 0.2501, 0.004), 9)
+    rng = np.random.default_rng(5)
+    sizes = [700, 512, 301, 900]                       # rows per group (ragged)
+    nt = sum(sizes)
+    fb = rng.integers(0, 64, size=(ndm, nt, nch)).astype(np.float32)
+    ref = oracle_incoherent(p, fb, ddm, nchan, ndec)
+    q = cdmt.cdmt_incoherent_query(plan, ddm, nt)
+    R, nfine, nout = q["shift_range"], len(ddm), q["nt_out"]
+    assert 0 < R and 2 * R <= min(sizes)
+    wrows = R + max(sizes)
+    win = torch.zeros((ndm, wrows, nch), dtype=torch.float32, device="cuda")
+    d_ts = torch.full((ndm, nfine, nout), -7.0, dtype=torch.float32, device="cuda")
+    ws = torch.empty(max(256, q["workspace_bytes"]), dtype=torch.uint8, device="cuda")
+    d_fb = torch.from_numpy(fb).cuda()
+    row0, done = 0, 0
+    for i, n in enumerate(sizes):
+        win[:, R:R + n] = d_fb[:, row0:row0 + n]        # stands for cdmt_execute writing the group's rows
+        first = i == 0
+        src = win[:, R:] if first else win
+        nt_in = n if first else R + n
+        cdmt.cdmt_incoherent_dedisperse(plan, src.data_ptr(), wrows * nch, nt_in, ddm, d_ts.data_ptr() + 4 * done,
+                                        nfine * nout, nout, ws, ws.numel())
+        done += nt_in - R
+        # the window's last R rows (rows [R + n - R, R + n) of the buffer) become its first
+        cdmt.cdmt_incoherent_carry(plan, win, wrows * nch, R + n, R)
+        row0 += n
+    torch.cuda.synchronize()
+    assert done == nout
+    got = d_ts.cpu().numpy()
+    for d in range(ndm):
+        assert np.array_equal(got[d], ref[d]["ts"]), d
+    bf, pf = cdmt.cdmt_incoherent_work(plan, ddm, nt)
+    assert bf == ndm * nfine * nch * nout and pf > 0
+
+
 def test_incoherent_argument_checks(cdmt):
     plan, _ = make_plan(cdmt, 2, 8, 1, 1)
     fb = torch.zeros((1, 400, 16), dtype=torch.float32, device="cuda")
