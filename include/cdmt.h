@@ -316,6 +316,40 @@ int cdmt_suggest_sizes(int nsub, const double *fcen_mhz, double bw_mhz, int ncha
                        double dm_max_abs, int chirp_ref, double min_efficiency, int *nfft,
                        int *noverlap);
 
+/*
+ * Per-group sizes inside the library (PAPER.md:79 fixes one N_bin and n_d for all subbands; PAPER.md:175
+ * names that as the program's inefficiency next to digifil, which "optimizes the choice for FFT size and
+ * data overlap ... depending on the DM and observing frequency").  A multiplan cuts the subbands (ascending
+ * fcen_mhz) into at most max_groups contiguous groups.  nfft is chosen as the paper chooses it -- by
+ * cdmt_suggest_sizes(min_efficiency) for the lowest subband at the largest |DM| -- and kept for every
+ * group (the same kernels run everywhere); a group takes the overlap Eq. 2 asks for at ITS lowest
+ * subband, and the cuts are those that keep most of the input (minimum of sum_g nsub_g noverlap_g over
+ * all contiguous partitions).  cdmt_multiplan_execute runs the groups one after the other (one workspace) into ONE filterbank
+ * d_out[ndm][nout_alloc][nsub*nchan] (descending frequency, plane stride out_stride_dm >= nout_alloc *
+ * nsub*nchan).  Common time grid: group g starts reading at input sample first_sample_g = max_h(noverlap_h/2)
+ * - noverlap_g/2, so row 0 of every group is the output sample that starts at input sample
+ * max_h(noverlap_h/2); group g fills rows [0, nout_g) of its columns, nout_g = nblock_g * Vd_g with its own
+ * block length; nout_valid = min_g nout_g rows are complete in every column, rows beyond nout_g of a group's
+ * columns are left untouched.  Results of group g are those of a plan made of its subbands and sizes, run on
+ * the input from first_sample_g on (same kernels, same bits).
+ * cdmt_multiplan_query / _group: host arithmetic; any output pointer may be NULL; kept_fraction = the
+ * subband-weighted (nfft - noverlap) / nfft.  Same alignment rules and errors as cdmt_execute.
+ */
+typedef struct cdmt_multiplan cdmt_multiplan; /* opaque */
+int cdmt_multiplan_create(cdmt_multiplan **mplan, int nsub, const double *fcen_mhz, double bw_mhz, int nchan,
+                          int ndec, int ndm, const double *dm, int in_dtype, int chirp_ref,
+                          double min_efficiency, int max_groups);
+int cdmt_multiplan_destroy(cdmt_multiplan *mplan);
+int cdmt_multiplan_query(const cdmt_multiplan *mplan, long long nsamp, int *ngroups, long long *nout_valid,
+                         long long *nout_alloc, size_t *out_bytes, size_t *workspace_bytes,
+                         double *kept_fraction);
+int cdmt_multiplan_group(const cdmt_multiplan *mplan, int group, long long nsamp, int *first_subband, int *nsub,
+                         int *nfft, int *noverlap, long long *first_sample, long long *nout);
+int cdmt_multiplan_execute(cdmt_multiplan *mplan, const void *d_in, long long nsamp, long long in_stride_pol,
+                           float *d_out, long long out_stride_dm, void *d_workspace, size_t workspace_bytes,
+                           void *cuda_stream);
+long long cdmt_multiplan_last_launch_count(const cdmt_multiplan *mplan);
+
 /* Measure the FP32 FMA rate of the device the stream belongs to (the "alu" roofline
  * denominator): runs `iters` dependent-chain FMA launches and returns
  * TFLOP/s in *tflops.  d_scratch: >= 4 bytes * 148 * 1024. */

@@ -32,6 +32,8 @@ EXPORTS = [
     "cdmt_forward_spectrum", "cdmt_redigitize", "cdmt_redigitize_sums", "cdmt_redigitize_workspace_bytes",
     "cdmt_incoherent_query", "cdmt_incoherent_shifts", "cdmt_incoherent_dedisperse", "cdmt_incoherent_carry", "cdmt_incoherent_work",
     "cdmt_sweep_seconds", "cdmt_min_overlap", "cdmt_suggest_sizes",
+    "cdmt_multiplan_create", "cdmt_multiplan_destroy", "cdmt_multiplan_query", "cdmt_multiplan_group",
+    "cdmt_multiplan_execute", "cdmt_multiplan_last_launch_count",
     "cdmt_measure_fp32_peak", "cdmt_last_launch_count", "cdmt_profile_read", "cdmt_strerror",
     "cdmt_version",
 ]
@@ -72,6 +74,15 @@ _lib.cdmt_incoherent_work.argtypes = [_vp, _i, C.POINTER(_d), _ll, C.POINTER(_d)
 _lib.cdmt_sweep_seconds.argtypes = [_d, _d, _d]
 _lib.cdmt_sweep_seconds.restype = _d
 _lib.cdmt_suggest_sizes.argtypes = [_i, C.POINTER(_d), _d, _i, _i, _d, _i, _d, C.POINTER(_i), C.POINTER(_i)]
+_lib.cdmt_multiplan_create.argtypes = [C.POINTER(_vp), _i, C.POINTER(_d), _d, _i, _i, _i, C.POINTER(_d), _i, _i, _d, _i]
+_lib.cdmt_multiplan_destroy.argtypes = [_vp]
+_lib.cdmt_multiplan_query.argtypes = [_vp, _ll, C.POINTER(_i), C.POINTER(_ll), C.POINTER(_ll), C.POINTER(_sz),
+                                      C.POINTER(_sz), C.POINTER(_d)]
+_lib.cdmt_multiplan_group.argtypes = [_vp, _i, _ll, C.POINTER(_i), C.POINTER(_i), C.POINTER(_i), C.POINTER(_i),
+                                      C.POINTER(_ll), C.POINTER(_ll)]
+_lib.cdmt_multiplan_execute.argtypes = [_vp, _vp, _ll, _ll, _vp, _ll, _vp, _sz, _vp]
+_lib.cdmt_multiplan_last_launch_count.argtypes = [_vp]
+_lib.cdmt_multiplan_last_launch_count.restype = _ll
 _lib.cdmt_min_overlap.argtypes = [_vp]
 _lib.cdmt_min_overlap.restype = _ll
 _lib.cdmt_measure_fp32_peak.argtypes = [_vp, _sz, _i, C.POINTER(_d), _vp]
@@ -313,6 +324,64 @@ def cdmt_suggest_sizes(fcen_mhz, bw_mhz: float, nchan: int, ndec: int, dm_max_ab
                                    float(dm_max_abs), int(chirp_ref), float(min_efficiency), C.byref(nfft),
                                    C.byref(nov)), "cdmt_suggest_sizes")
     return nfft.value, nov.value
+
+
+class MultiPlan:
+    """Owner of a cdmt_multiplan*."""
+
+    def __init__(self, handle: int, nsub, nchan, ndec, ndm, in_dtype):
+        self.handle = handle
+        self.nsub, self.nchan, self.ndec, self.ndm, self.in_dtype = nsub, nchan, ndec, ndm, in_dtype
+
+    def __del__(self):
+        if getattr(self, "handle", None) and _lib is not None:
+            _lib.cdmt_multiplan_destroy(self.handle)
+            self.handle = None
+
+
+def cdmt_multiplan_create(nsub, fcen_mhz, bw_mhz, nchan, ndec, dm, in_dtype=IN_CF32, chirp_ref=REF_CHANNEL,
+                          min_efficiency=0.9, max_groups=4) -> MultiPlan:
+    fc = np.ascontiguousarray(fcen_mhz, dtype=np.float64).reshape(-1)
+    dms = np.ascontiguousarray(dm, dtype=np.float64).reshape(-1)
+    h = _vp()
+    st = _lib.cdmt_multiplan_create(C.byref(h), int(nsub), fc.ctypes.data_as(C.POINTER(_d)), float(bw_mhz), int(nchan),
+                                    int(ndec), int(dms.size), dms.ctypes.data_as(C.POINTER(_d)), int(in_dtype),
+                                    int(chirp_ref), float(min_efficiency), int(max_groups))
+    _check(st, "cdmt_multiplan_create")
+    return MultiPlan(h.value, int(nsub), int(nchan), int(ndec), int(dms.size), int(in_dtype))
+
+
+def cdmt_multiplan_destroy(mp: MultiPlan):
+    if mp.handle:
+        _check(_lib.cdmt_multiplan_destroy(mp.handle), "cdmt_multiplan_destroy")
+        mp.handle = None
+
+
+def cdmt_multiplan_query(mp: MultiPlan, nsamp: int) -> dict:
+    ng, nv, na, ob, wb, kf = _i(), _ll(), _ll(), _sz(), _sz(), _d()
+    _check(_lib.cdmt_multiplan_query(mp.handle, int(nsamp), C.byref(ng), C.byref(nv), C.byref(na), C.byref(ob),
+                                     C.byref(wb), C.byref(kf)), "cdmt_multiplan_query")
+    return dict(ngroups=ng.value, nout_valid=nv.value, nout_alloc=na.value, out_bytes=ob.value,
+                workspace_bytes=wb.value, kept_fraction=kf.value)
+
+
+def cdmt_multiplan_group(mp: MultiPlan, group: int, nsamp: int) -> dict:
+    s0, ns, nf, no, fs, nr = _i(), _i(), _i(), _i(), _ll(), _ll()
+    _check(_lib.cdmt_multiplan_group(mp.handle, int(group), int(nsamp), C.byref(s0), C.byref(ns), C.byref(nf),
+                                     C.byref(no), C.byref(fs), C.byref(nr)), "cdmt_multiplan_group")
+    return dict(first_subband=s0.value, nsub=ns.value, nfft=nf.value, noverlap=no.value, first_sample=fs.value,
+                nout=nr.value)
+
+
+def cdmt_multiplan_execute(mp: MultiPlan, d_in, nsamp: int, in_stride_pol: int, d_out, out_stride_dm: int,
+                           d_workspace, workspace_bytes: int, stream=None):
+    st = _lib.cdmt_multiplan_execute(mp.handle, _ptr(d_in), int(nsamp), int(in_stride_pol), _ptr(d_out),
+                                     int(out_stride_dm), _ptr(d_workspace), int(workspace_bytes), _stream(stream))
+    _check(st, "cdmt_multiplan_execute")
+
+
+def cdmt_multiplan_last_launch_count(mp: MultiPlan) -> int:
+    return _lib.cdmt_multiplan_last_launch_count(mp.handle)
 
 
 def cdmt_last_launch_count(plan: Plan) -> int:

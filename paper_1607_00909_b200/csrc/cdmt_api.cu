@@ -1,5 +1,6 @@
 // cdmt_api.cu -- the C ABI declared in include/cdmt.h: plan bookkeeping (host only) and the
 // launch sequences.  No arithmetic of the method lives here except the Eq. 2 helper.
+#include <algorithm>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -289,7 +290,7 @@ static int validate_input(const cdmt_plan *plan, const void *d_in, long long nsa
 
 static int run_chunks(cdmt_plan *plan, const void *d_in, long long in_stride_pol, long long nb, float *d_out,
                       long long out_stride_dm, float2 *d_spec_out, void *d_workspace, size_t workspace_bytes,
-                      cudaStream_t st, double *d_segsum = nullptr)
+                      cudaStream_t st, double *d_segsum = nullptr, int out_pitch = 0)
 {
     const Geometry &g = plan->g;
     const long long nunits = nb * g.nsub;
@@ -334,7 +335,7 @@ static int run_chunks(cdmt_plan *plan, const void *d_in, long long in_stride_pol
         if (profile) plan->spans.push_back({a, b, 0});
         if (d_out) {
             bool chunk_sums = true;
-            rc = check_cuda(launch_fused(g, ws, spec, (int)u0, n, d_out, out_stride_dm, plan->dm_tile,
+            rc = check_cuda(launch_fused(g, ws, spec, (int)u0, n, d_out, out_stride_dm, out_pitch, plan->dm_tile,
                                          plan->accurate, plan->force_generic, plan->dm.data(),
                                          plan->fcen.data(), d_segsum, (int)nb, &chunk_sums, st,
                                          &plan->last_launches));
@@ -752,7 +753,7 @@ static int plan_incoherent(cdmt_plan *plan, int nfine, const double *ddm)
         plan->ic_ddm.clear();
         if (!incoherent_plan(plan->g, plan->fcen.data(), nfine, ddm, &plan->ic)) return CDMT_ERR_ARG;
         // shift range beyond the shared-memory tile, or more trial groups than a grid dimension holds
-        if (!incoherent_config(plan->ic, nullptr, nullptr, nullptr)) return CDMT_ERR_SIZE;
+        if (!incoherent_config(plan->ic, nullptr, nullptr, nullptr, nullptr, nullptr)) return CDMT_ERR_SIZE;
         plan->ic_ddm.assign(ddm, ddm + nfine);
     } catch (...) {
         plan->ic_ddm.clear();
@@ -903,6 +904,210 @@ extern "C" int cdmt_suggest_sizes(int nsub, const double *fcen_mhz, double bw_mh
     }
     return CDMT_ERR_SIZE;
 }
+
+// ---- per-group sizes inside the library (N4) ------------------------------------------------
+// PAPER.md:79 fixes one (N_bin, n_d) for all subbands, "chosen for the lowest observing frequency of the
+// input data and highest DM", and names that as the program's own inefficiency next to
+// digifil.  A multiplan cuts the subbands into contiguous groups, sizes each from Eq. 2 (cdmt_suggest_sizes)
+// and runs them one after the other into ONE filterbank: every group starts reading its input at the sample
+// that puts its first output sample at the same time as the others', so the rows line up.
+struct cdmt_multiplan {
+    std::vector<cdmt_plan *> plans;      // one per group, ascending frequency
+    std::vector<int> sub0, nsubg;        // subband range of each group
+    int nsub, nchan, ndec, ndm, in_dtype;
+    long long last_launches;
+};
+
+struct MultiSizes {
+    std::vector<long long> delta, nblock, rows;   // first input sample, blocks and output rows of each group
+    long long rows_valid, rows_alloc;
+    size_t workspace;
+    double kept;                                  // kept fraction of the input, subband-weighted
+};
+
+static int multi_sizes(const cdmt_multiplan *mp, long long nsamp, MultiSizes *z)
+{
+    const size_t ng = mp->plans.size();
+    long long tstart = 0;
+    for (const cdmt_plan *p : mp->plans) tstart = std::max<long long>(tstart, p->g.noverlap / 2);
+    z->delta.resize(ng); z->nblock.resize(ng); z->rows.resize(ng);
+    z->rows_valid = -1; z->rows_alloc = 0; z->workspace = 0; z->kept = 0.0;
+    for (size_t i = 0; i < ng; ++i) {
+        const cdmt_plan *p = mp->plans[i];
+        const Geometry &g = p->g;
+        z->delta[i] = tstart - g.noverlap / 2;
+        const long long nb = nblock_for(g, nsamp - z->delta[i]);
+        if (nb < 1 || nb * g.nsub > (1LL << 30)) return CDMT_ERR_SIZE;
+        z->nblock[i] = nb;
+        z->rows[i] = nb * g.vdec;
+        z->rows_valid = z->rows_valid < 0 ? z->rows[i] : std::min(z->rows_valid, z->rows[i]);
+        z->rows_alloc = std::max(z->rows_alloc, z->rows[i]);
+        const long long cu = chunk_units_for(p, nb * g.nsub);
+        z->workspace = std::max(z->workspace, workspace_layout(g, (int)cu, nullptr, nullptr));
+        z->kept += (double)g.nsub * (double)g.step / (double)g.nfft;
+    }
+    z->kept /= (double)mp->nsub;
+    return CDMT_OK;
+}
+
+extern "C" int cdmt_multiplan_destroy(cdmt_multiplan *mp)
+{
+    if (!mp) return CDMT_ERR_ARG;
+    for (cdmt_plan *p : mp->plans) cdmt_plan_destroy(p);
+    delete mp;
+    return CDMT_OK;
+}
+
+extern "C" int cdmt_multiplan_create(cdmt_multiplan **mplan, int nsub, const double *fcen_mhz, double bw_mhz, int nchan,
+                                     int ndec, int ndm, const double *dm, int in_dtype, int chirp_ref,
+                                     double min_efficiency, int max_groups)
+{
+    if (!mplan) return CDMT_ERR_ARG;
+    *mplan = nullptr;
+    if (!fcen_mhz || !dm || nsub < 1 || ndm < 1 || max_groups < 1) return CDMT_ERR_ARG;
+    for (int s = 1; s < nsub; ++s)
+        if (!(fcen_mhz[s] > fcen_mhz[s - 1])) return CDMT_ERR_ARG;   // groups are contiguous in frequency
+    double dmax = 0.0;
+    for (int d = 0; d < ndm; ++d) {
+        if (!std::isfinite(dm[d])) return CDMT_ERR_ARG;
+        dmax = std::max(dmax, std::fabs(dm[d]));
+    }
+    try {
+        // nfft as the paper chooses it: from the lowest subband at the largest DM.  Every group
+        // keeps that nfft (the same kernels run everywhere) and takes the overlap Eq. 2 asks for at ITS lowest
+        // subband; the cuts are the ones that keep most of the input: minimise sum_g n_g noverlap_g over all
+        // partitions into at most max_groups contiguous groups (dynamic programme over the subbands).
+        int nfft0 = 0, nov0 = 0;
+        int rc0 = cdmt_suggest_sizes(nsub, fcen_mhz, bw_mhz, nchan, ndec, dmax, chirp_ref, min_efficiency, &nfft0, &nov0);
+        if (rc0) return rc0;
+        std::vector<int> nov((size_t)nsub);
+        for (int s = 0; s < nsub; ++s) {
+            int nf = 0;
+            rc0 = cdmt_suggest_sizes(1, fcen_mhz + s, bw_mhz, nchan, ndec, dmax, chirp_ref, 1e-6, &nf, &nov[s]);
+            if (rc0) return rc0;
+        }
+        struct Grp { int s0, n, nfft, nov; };
+        std::vector<Grp> grp;
+        const int G = std::min(max_groups, nsub);
+        if (nsub > 8192) {
+            // very wide bands: even cuts (the programme above is quadratic in nsub)
+            for (int g = 0; g < G; ++g) {
+                const int a = (int)((long long)nsub * g / G), b = (int)((long long)nsub * (g + 1) / G);
+                grp.push_back({a, b - a, nfft0, nov[a]});
+            }
+        } else {
+            const double INF = 1e300;
+            std::vector<std::vector<double>> cost((size_t)G + 1, std::vector<double>((size_t)nsub + 1, INF));
+            std::vector<std::vector<int>> from((size_t)G + 1, std::vector<int>((size_t)nsub + 1, -1));
+            cost[0][0] = 0.0;
+            for (int g = 1; g <= G; ++g)
+                for (int j = 1; j <= nsub; ++j)
+                    for (int i = g - 1; i < j; ++i) {
+                        if (cost[g - 1][i] >= INF) continue;
+                        const double c = cost[g - 1][i] + (double)(j - i) * (double)nov[i];
+                        if (c < cost[g][j]) { cost[g][j] = c; from[g][j] = i; }
+                    }
+            int gbest = 1;
+            for (int g = 2; g <= G; ++g)
+                if (cost[g][nsub] < cost[gbest][nsub]) gbest = g;
+            std::vector<int> cuts;
+            for (int g = gbest, j = nsub; g >= 1; --g) {
+                cuts.push_back(from[g][j]);
+                j = from[g][j];
+            }
+            std::reverse(cuts.begin(), cuts.end());
+            for (size_t k = 0; k < cuts.size(); ++k) {
+                const int a = cuts[k], b = k + 1 < cuts.size() ? cuts[k + 1] : nsub;
+                if (!grp.empty() && nov[a] == grp.back().nov) grp.back().n += b - a;   // same overlap: one group
+                else grp.push_back({a, b - a, nfft0, nov[a]});
+            }
+        }
+        cdmt_multiplan *mp = new cdmt_multiplan();
+        mp->nsub = nsub; mp->nchan = nchan; mp->ndec = ndec; mp->ndm = ndm; mp->in_dtype = in_dtype; mp->last_launches = 0;
+        for (const Grp &g : grp) {
+            cdmt_plan *p = nullptr;
+            const int rc = cdmt_plan_create(&p, g.n, fcen_mhz + g.s0, bw_mhz, g.nfft, g.nov, nchan, ndec, ndm, dm, in_dtype,
+                                            chirp_ref);
+            if (rc) {
+                cdmt_multiplan_destroy(mp);
+                return rc;
+            }
+            mp->plans.push_back(p);
+            mp->sub0.push_back(g.s0);
+            mp->nsubg.push_back(g.n);
+        }
+        *mplan = mp;
+    } catch (...) {
+        return CDMT_ERR_ALLOC;
+    }
+    return CDMT_OK;
+}
+
+extern "C" int cdmt_multiplan_query(const cdmt_multiplan *mp, long long nsamp, int *ngroups, long long *nout_valid,
+                                    long long *nout_alloc, size_t *out_bytes, size_t *workspace_bytes,
+                                    double *kept_fraction)
+{
+    if (!mp) return CDMT_ERR_ARG;
+    MultiSizes z;
+    const int rc = multi_sizes(mp, nsamp, &z);
+    if (rc) return rc;
+    if (ngroups) *ngroups = (int)mp->plans.size();
+    if (nout_valid) *nout_valid = z.rows_valid;
+    if (nout_alloc) *nout_alloc = z.rows_alloc;
+    if (out_bytes) *out_bytes = (size_t)mp->ndm * (size_t)z.rows_alloc * (size_t)mp->nsub * mp->nchan * sizeof(float);
+    if (workspace_bytes) *workspace_bytes = z.workspace;
+    if (kept_fraction) *kept_fraction = z.kept;
+    return CDMT_OK;
+}
+
+extern "C" int cdmt_multiplan_group(const cdmt_multiplan *mp, int group, long long nsamp, int *first_subband, int *nsub,
+                                    int *nfft, int *noverlap, long long *first_sample, long long *nout)
+{
+    if (!mp || group < 0 || group >= (int)mp->plans.size()) return CDMT_ERR_ARG;
+    MultiSizes z;
+    const int rc = multi_sizes(mp, nsamp, &z);
+    if (rc) return rc;
+    const Geometry &g = mp->plans[group]->g;
+    if (first_subband) *first_subband = mp->sub0[group];
+    if (nsub) *nsub = g.nsub;
+    if (nfft) *nfft = g.nfft;
+    if (noverlap) *noverlap = g.noverlap;
+    if (first_sample) *first_sample = z.delta[group];
+    if (nout) *nout = z.rows[group];
+    return CDMT_OK;
+}
+
+extern "C" int cdmt_multiplan_execute(cdmt_multiplan *mp, const void *d_in, long long nsamp, long long in_stride_pol,
+                                      float *d_out, long long out_stride_dm, void *d_workspace, size_t workspace_bytes,
+                                      void *cuda_stream)
+{
+    if (!mp || !d_in || !d_out || !d_workspace) return CDMT_ERR_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_workspace) & 255) != 0 || (reinterpret_cast<uintptr_t>(d_out) & 3) != 0)
+        return CDMT_ERR_ARG;
+    const uintptr_t word = mp->in_dtype == CDMT_IN_CI8 ? 2 : 8;
+    if ((reinterpret_cast<uintptr_t>(d_in) & (word - 1)) != 0) return CDMT_ERR_ARG;
+    if (in_stride_pol < nsamp) return CDMT_ERR_SIZE;
+    MultiSizes z;
+    int rc = multi_sizes(mp, nsamp, &z);
+    if (rc) return rc;
+    const long long pitch = (long long)mp->nsub * mp->nchan;
+    if (pitch > 0x7fffffffLL || out_stride_dm < z.rows_alloc * pitch) return CDMT_ERR_SIZE;
+    if (workspace_bytes < z.workspace) return CDMT_ERR_WORKSPACE;
+    mp->last_launches = 0;
+    for (size_t i = 0; i < mp->plans.size(); ++i) {
+        cdmt_plan *p = mp->plans[i];
+        const char *in = static_cast<const char *>(d_in) + ((size_t)2 * mp->sub0[i] * (size_t)in_stride_pol + (size_t)z.delta[i]) * word;
+        // descending frequency: the highest group comes first in a row
+        float *out = d_out + (size_t)(mp->nsub - mp->sub0[i] - mp->nsubg[i]) * mp->nchan;
+        rc = run_chunks(p, in, in_stride_pol, z.nblock[i], out, out_stride_dm, nullptr, d_workspace, workspace_bytes,
+                        static_cast<cudaStream_t>(cuda_stream), nullptr, (int)pitch);
+        mp->last_launches += p->last_launches;
+        if (rc) return rc;
+    }
+    return CDMT_OK;
+}
+
+extern "C" long long cdmt_multiplan_last_launch_count(const cdmt_multiplan *mp) { return mp ? mp->last_launches : -1; }
 
 extern "C" long long cdmt_last_launch_count(const cdmt_plan *plan) { return plan ? plan->last_launches : -1; }
 

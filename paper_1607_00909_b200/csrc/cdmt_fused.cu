@@ -81,7 +81,7 @@ __global__ void __launch_bounds__(M / 16) k_fused_generic(const FusedArgs a)
 #pragma unroll
             for (int i = 0; i < 16; ++i) acc[i] = fmaf(v[i].x, v[i].x, fmaf(v[i].y, v[i].y, acc[i]));
         }
-        float *outd = a.out + (size_t)d * (size_t)a.out_stride_dm + (size_t)b * a.vdec * nchan_total + ochan;
+        float *outd = a.out + (size_t)d * (size_t)a.out_stride_dm + (size_t)b * a.vdec * a.out_pitch + ochan;
         float *I = reinterpret_cast<float *>(ex);
         __syncthreads();
 #pragma unroll
@@ -92,7 +92,7 @@ __global__ void __launch_bounds__(M / 16) k_fused_generic(const FusedArgs a)
         for (int qd = tid; qd < a.vdec; qd += NT) {
             float sum = 0.f;
             for (int r = 0; r < a.ndec; ++r) sum += I[a.hdisc + qd * a.ndec + r];
-            outd[(size_t)qd * nchan_total] = sum * a.scale;
+            outd[(size_t)qd * a.out_pitch] = sum * a.scale;
         }
     }
 }
@@ -261,7 +261,7 @@ k_fused_fast(const FusedArgs a, const __grid_constant__ DmParams dmp)
     }
     const int nchan_total = a.nsub * a.nchan;
     const int ochan = nchan_total - 1 - (s * a.nchan + c);
-    float *out0 = a.out + (size_t)b * a.vdec * nchan_total + ochan;
+    float *out0 = a.out + (size_t)b * a.vdec * a.out_pitch + ochan;
     const int d_begin = a.dm_first + blockIdx.y * a.dm_tile;
     const int d_end = min(a.ndm, d_begin + a.dm_tile);
     // pass-0 thread (rho, d1) = (tid >> 4, tid & 15) stores at rho*RHO + d1*PITCH + 0..15
@@ -321,7 +321,7 @@ k_fused_fast(const FusedArgs a, const __grid_constant__ DmParams dmp)
             const int n = (lane & ((1 << LS) - 1)) + (1 << LS) * j;
             const int t0 = (tid & ~(D - 1)) + NT * n;  // first sample of the integrated group
             if ((lane & (D - 1)) < (1 << LS) && t0 >= a.hdisc && t0 < M - a.hdisc)
-                outd[(size_t)((t0 - a.hdisc) >> LOGD) * nchan_total] = res[j] * a.scale;
+                outd[(size_t)((t0 - a.hdisc) >> LOGD) * a.out_pitch] = res[j] * a.scale;
         }
     }
 }
@@ -402,7 +402,7 @@ static double phase_cycles_bound(const Geometry &g, const double *h_dm, const do
 }
 
 cudaError_t launch_fused(const Geometry &g, const Workspace &ws, const float2 *spec, int unit0, int nunits,
-                         float *d_out, long long out_stride_dm, int dm_tile, int accurate, int force_generic,
+                         float *d_out, long long out_stride_dm, int out_pitch, int dm_tile, int accurate, int force_generic,
                          const double *h_dm, const double *h_fcen, double *d_segsum, int nblock_total,
                          bool *sums_done, cudaStream_t st, long long *launches)
 {
@@ -412,7 +412,7 @@ cudaError_t launch_fused(const Geometry &g, const Workspace &ws, const float2 *s
     dim3 grid((unsigned)(nunits * g.nchan), (unsigned)((g.ndm + dm_tile - 1) / dm_tile));
     FusedArgs fa;
     fa.spec = spec; fa.tw = ws.tw_m; fa.dmlist = ws.dm; fa.fcen = ws.fcen; fa.out = d_out;
-    fa.out_stride_dm = out_stride_dm; fa.unit0 = unit0; fa.nsub = g.nsub; fa.nchan = g.nchan; fa.nfft = g.nfft;
+    fa.out_stride_dm = out_stride_dm; fa.out_pitch = out_pitch > 0 ? out_pitch : g.nsub * g.nchan; fa.unit0 = unit0; fa.nsub = g.nsub; fa.nchan = g.nchan; fa.nfft = g.nfft;
     fa.hdisc = g.hdisc; fa.ndec = g.ndec; fa.vdec = g.vdec; fa.ndm = g.ndm; fa.dm_tile = dm_tile;
     fa.chirp_ref = g.chirp_ref; fa.accurate = accurate; fa.bw_mhz = g.bw_mhz;
     fa.scale = (float)(1.0 / ((double)g.nfft * (double)M));

@@ -208,7 +208,7 @@ k_fused_x2(const FusedArgs a, const __grid_constant__ DmParams dmp)
     }
     const int nchan_total = a.nsub * a.nchan;
     const int ochan = nchan_total - 1 - (s * a.nchan + c);
-    float *out0 = a.out + (size_t)b * a.vdec * nchan_total + ochan;
+    float *out0 = a.out + (size_t)b * a.vdec * a.out_pitch + ochan;
     const int d_begin = a.dm_first + blockIdx.y * a.dm_tile;
     const int d_end = min(a.ndm, d_begin + a.dm_tile);
     float2 *ib = integ + warp * G::INTEG;
@@ -330,9 +330,9 @@ k_fused_x2(const FusedArgs a, const __grid_constant__ DmParams dmp)
             }
             const int t0 = tgrp + NT * n;
             if (D <= 16 || lane < 16) {
-                if (t0 >= a.hdisc && t0 < M - a.hdisc) outd[(size_t)((t0 - a.hdisc) >> LOGD) * nchan_total] = s0 * a.scale;
+                if (t0 >= a.hdisc && t0 < M - a.hdisc) outd[(size_t)((t0 - a.hdisc) >> LOGD) * a.out_pitch] = s0 * a.scale;
                 const int t1 = t0 + L;
-                if (t1 >= a.hdisc && t1 < M - a.hdisc) outd[(size_t)((t1 - a.hdisc) >> LOGD) * nchan_total] = s1 * a.scale;
+                if (t1 >= a.hdisc && t1 < M - a.hdisc) outd[(size_t)((t1 - a.hdisc) >> LOGD) * a.out_pitch] = s1 * a.scale;
             }
         }
     }

@@ -177,7 +177,7 @@ k_fused_sp(const FusedArgs a, const __grid_constant__ DmParams dmp)
     }
     const int nchan_total = a.nsub * a.nchan;
     const int ochan = nchan_total - 1 - (s * a.nchan + c);
-    float *out0 = a.out + (size_t)b * a.vdec * nchan_total + ochan;
+    float *out0 = a.out + (size_t)b * a.vdec * a.out_pitch + ochan;
     const int d_begin = a.dm_first + blockIdx.y * a.dm_tile;
     const int d_end = min(a.ndm, d_begin + a.dm_tile);
     float4 *const p0 = ex + j2 * G::RHO + j1 * G::PITCH;   // pass-0 stores: [t0]
@@ -274,7 +274,7 @@ k_fused_sp(const FusedArgs a, const __grid_constant__ DmParams dmp)
             const int n = (lane & ((1 << LS) - 1)) + (1 << LS) * j;
             const int t0 = (tid & ~(D - 1)) + NT * n;  // first sample of the integrated group
             if ((lane & (D - 1)) < (1 << LS) && t0 >= a.hdisc && t0 < M - a.hdisc)
-                outd[(size_t)((t0 - a.hdisc) >> LOGD) * nchan_total] = pw[j] * a.scale;
+                outd[(size_t)((t0 - a.hdisc) >> LOGD) * a.out_pitch] = pw[j] * a.scale;
         }
     }
     tmem_fence_before_sync();

@@ -301,7 +301,7 @@ k_fused_ws(const FusedArgs a, const __grid_constant__ DmParams dmp)
         if (active) {
             const int nchan_total = a.nsub * a.nchan;
             const int ochan = nchan_total - 1 - (s * a.nchan + c);
-            float *out0 = a.out + (size_t)b * a.vdec * nchan_total + ochan;
+            float *out0 = a.out + (size_t)b * a.vdec * a.out_pitch + ochan;
             const int il = lane & (DG - 1), g0 = lane - il;
             const int tgrp = (D > 16) ? (t & ~31) : (t - il);  // first sample of a lane's group, before + NT n
 
@@ -331,13 +331,13 @@ k_fused_ws(const FusedArgs a, const __grid_constant__ DmParams dmp)
                     if (D <= 16 || lane < 16) {
                         if (t0 >= a.hdisc && t0 < M - a.hdisc) {
                             const float f = s0 * a.scale;
-                            outd[(size_t)((t0 - a.hdisc) >> LOGD) * nchan_total] = f;
+                            outd[(size_t)((t0 - a.hdisc) >> LOGD) * a.out_pitch] = f;
                             mine[(2 * kk) & 3] = f;
                         }
                         const int t1 = t0 + L;
                         if (t1 >= a.hdisc && t1 < M - a.hdisc) {
                             const float f = s1 * a.scale;
-                            outd[(size_t)((t1 - a.hdisc) >> LOGD) * nchan_total] = f;
+                            outd[(size_t)((t1 - a.hdisc) >> LOGD) * a.out_pitch] = f;
                             mine[(2 * kk + 1) & 3] = f;
                         }
                     }

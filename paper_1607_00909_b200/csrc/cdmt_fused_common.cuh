@@ -46,6 +46,7 @@ struct FusedArgs {
     const double *fcen;
     float *out;
     long long out_stride_dm;
+    int out_pitch;           // elements between consecutive time samples of `out` (>= nsub * nchan)
     int unit0, nsub, nchan, nfft, hdisc, ndec, vdec, ndm, dm_tile, chirp_ref, accurate;
     int dm_first, dm_param0;  // DM range [dm_first, ndm) of this launch; dmp.dm[0] is trial dm_param0
     int nb_chunk;             // k_fused_ws: whole blocks in this chunk (units = nb_chunk * nsub)

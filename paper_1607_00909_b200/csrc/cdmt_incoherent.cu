@@ -122,6 +122,7 @@ struct IcArgs {
     const uint2 *entries;   // [ngroups][nch]
     const int2 *groups;     // [ngroups]
     int nt_in, nt_out, nch, ngroups, cc, tw, vec_in;
+    int gpc, tt;            // trial groups and 256-sample time tiles per CTA: gpc * tt <= IC_WARPS warps are live
 };
 
 // Run sums of the distinct shifts O1 and O2 = O1 + 1 of one channel: if spread >= O1 add this lane's
@@ -182,18 +183,24 @@ __device__ __forceinline__ void ic_run_add2(float (&PA)[8], float (&PB)[8], unsi
         : "memory");
 }
 
-// grid (ceil(nt_out / 256), ceil(ngroups / IC_WARPS), ndm), 32 IC_WARPS threads; dynamic shared memory:
-// float tile[cc][tw] and uint2 tab[IC_WARPS][cc]
+// grid (ceil(nt_out / (256 tt)), ceil(ngroups / gpc), ndm), 32 IC_WARPS threads; warp w works on trial group
+// w % gpc and time tile w / gpc of the CTA (few trial groups: several time tiles share one staged tile,
+// so that the warps stay busy and the halo is re-read less).  Dynamic shared memory: float tile[cc][tw]
+// and uint2 tab[gpc][cc]
+template <bool MULTI>   // false: gpc = IC_WARPS, tt = 1 as compile-time constants (the common, register-tight case)
 __global__ void __launch_bounds__(32 * IC_WARPS, 1) k_incoherent(const IcArgs a)
 {
+    const int gpc = MULTI ? a.gpc : IC_WARPS, tt = MULTI ? a.tt : 1;
     extern __shared__ float4 ic_smem4[];
     float *tile = reinterpret_cast<float *>(ic_smem4);
     const int cc = a.cc, tw = a.tw, quads = cc >> 2;
     uint2 *tab = reinterpret_cast<uint2 *>(tile + (((size_t)cc * tw + 3) & ~(size_t)3));
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int t0 = blockIdx.x * IC_TILE;
-    const int grp = blockIdx.y * IC_WARPS + warp;
-    const bool live = grp < a.ngroups;
+    const int tbase = blockIdx.x * IC_TILE * tt;           // first sample of the staged tile
+    const int gsel = MULTI ? warp % gpc : warp, sub = MULTI ? warp / gpc : 0;
+    const int t0 = tbase + sub * IC_TILE;                  // first output sample of this warp
+    const int grp = blockIdx.y * gpc + gsel;
+    const bool live = sub < tt && grp < a.ngroups && t0 < a.nt_out;
     const float *fb = a.fb + (size_t)blockIdx.z * (size_t)a.fb_stride_dm;
     const int rows = tw;                     // input samples staged per chunk
     const int rstep = (32 * IC_WARPS) / quads;
@@ -219,7 +226,7 @@ __global__ void __launch_bounds__(32 * IC_WARPS, 1) k_incoherent(const IcArgs a)
             float gq[4][4];
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                const int i = ib + u * rstep, t = t0 + i;
+                const int i = ib + u * rstep, t = tbase + i;
 #pragma unroll
                 for (int e = 0; e < 4; ++e) gq[u][e] = 0.f;
                 if (i < rows && t < a.nt_in) {
@@ -243,9 +250,9 @@ __global__ void __launch_bounds__(32 * IC_WARPS, 1) k_incoherent(const IcArgs a)
                 }
             }
         }
-        for (int e = tid; e < IC_WARPS * cc; e += 32 * IC_WARPS) {
+        for (int e = tid; e < gpc * cc; e += 32 * IC_WARPS) {
             const int w = e / cc, c = e % cc;
-            const int gw = blockIdx.y * IC_WARPS + w;
+            const int gw = blockIdx.y * gpc + w;
             uint2 v = make_uint2(0u, 0u);
             if (gw < a.ngroups && c0 + c < a.nch) v = a.entries[(size_t)gw * a.nch + c0 + c];
             tab[w * cc + c] = v;
@@ -255,13 +262,13 @@ __global__ void __launch_bounds__(32 * IC_WARPS, 1) k_incoherent(const IcArgs a)
         // ---- add the chunk's channels into the run sums; at the end of a run, into the trials
 #pragma unroll 1
         for (int c = 0; c < cc; ++c) {
-            const uint2 e0 = tab[warp * cc + c];
+            const uint2 e0 = tab[gsel * cc + c];
             // the table words are the same in every lane; the shuffles let the compiler know it
             uint2 e;
             e.x = __shfl_sync(0xffffffffu, e0.x, 0);
             e.y = __shfl_sync(0xffffffffu, e0.y, 0);
             const unsigned s0 = e.x & 0xffffffu, spread = (e.x >> 24) & 7u;
-            const float *p = tile + (size_t)c * tw + s0 + lane;
+            const float *p = tile + (size_t)c * tw + s0 + lane + sub * IC_TILE;
 #pragma unroll
             for (int i = 0; i < 8; ++i) P[0][i] += p[32 * i];
             const unsigned sp = (unsigned)__cvta_generic_to_shared(p);
@@ -332,26 +339,38 @@ cudaError_t launch_carry_rows(float *d_fb, long long fb_stride_dm, long long nt_
 }
 
 // ---------------------------------------------------------------------------------------- launch
-// Tile geometry for a shift range: the row length (>= range + 256 and = 1 mod 32) and the channels per
-// chunk that fit shared memory; false if even four channels do not fit (range > ~14000) or there are more
-// trial groups than a grid dimension holds.
-bool incoherent_config(const IncoherentTables &T, int *cc_out, int *tw_out, size_t *smem_out)
+// Launch geometry: trial groups and time tiles per CTA, the row length of the staged tile and the channels
+// per chunk that fit shared memory; false if even four channels of 256 + range samples do not fit
+// (range > ~14000) or there are more trial groups than a grid dimension holds.
+bool incoherent_config(const IncoherentTables &T, int *cc_out, int *tw_out, int *gpc_out, int *tt_out, size_t *smem_out)
 {
-    const int tw = ((T.range + IC_TILE + 30) & ~31) + 1;
-    auto smem_for = [&](int cc) { return sizeof(float) * (((size_t)cc * tw + 3) & ~(size_t)3) + sizeof(uint2) * IC_WARPS * cc; };
-    // channels per chunk: the largest of 32, 16, 8, 4 whose tile lets two CTAs share an SM, else whatever fits
-    int cc = 0;
-    for (int c : {32, 16, 8, 4})
-        if (smem_for(c) <= 72 * 1024) { cc = c; break; }
-    if (!cc)
-        for (int c : {32, 16, 8, 4})
-            if (smem_for(c) <= 227 * 1024) { cc = c; break; }
-    if (!cc) return false;
-    if ((T.groups.size() + IC_WARPS - 1) / IC_WARPS > 65535) return false;   // grid.y
-    if (cc_out) *cc_out = cc;
-    if (tw_out) *tw_out = tw;
-    if (smem_out) *smem_out = smem_for(cc);
-    return true;
+    const int ngroups = (int)T.groups.size();
+    if (ngroups < 1) return false;
+    // trial groups per CTA (balanced over grid.y) and, where they do not fill the warps, time tiles per CTA
+    const int ny = (ngroups + IC_WARPS - 1) / IC_WARPS;
+    if (ny > 65535) return false;
+    const int gpc = (ngroups + ny - 1) / ny;
+    int tt = IC_WARPS / gpc;
+    for (;; --tt) {
+        const int tw = ((T.range + tt * IC_TILE + 30) & ~31) + 1;   // >= range + 256 tt and = 1 mod 32
+        auto smem_for = [&](int cc) { return sizeof(float) * (((size_t)cc * tw + 3) & ~(size_t)3) + sizeof(uint2) * gpc * cc; };
+        // channels per chunk: 32 if the tile stays below 72 KB, else fewer time tiles; at one time tile
+        // whatever number of channels fits shared memory
+        int cc = 0;
+        if (smem_for(32) <= 72 * 1024) cc = 32;
+        else if (tt == 1)
+            for (int c : {32, 16, 8, 4})
+                if (smem_for(c) <= 227 * 1024) { cc = c; break; }
+        if (cc) {
+            if (cc_out) *cc_out = cc;
+            if (tw_out) *tw_out = tw;
+            if (gpc_out) *gpc_out = gpc;
+            if (tt_out) *tt_out = tt;
+            if (smem_out) *smem_out = smem_for(cc);
+            return true;
+        }
+        if (tt == 1) return false;   // even four channels of 256 + range samples do not fit
+    }
 }
 
 void incoherent_release(IncoherentTables *T)
@@ -388,12 +407,15 @@ cudaError_t launch_incoherent(const Geometry &g, IncoherentTables &T, const floa
     a.entries = d_entries; a.groups = d_groups;
     a.nt_in = (int)nt_in; a.nt_out = (int)nt_out; a.nch = nch; a.ngroups = ngroups;
     size_t smem = 0;
-    if (!incoherent_config(T, &a.cc, &a.tw, &smem)) return cudaErrorInvalidValue;
+    if (!incoherent_config(T, &a.cc, &a.tw, &a.gpc, &a.tt, &smem)) return cudaErrorInvalidValue;
     a.vec_in = (nch % 4 == 0 && fb_stride_dm % 4 == 0 && (reinterpret_cast<uintptr_t>(d_fb) & 15) == 0) ? 1 : 0;
-    e = cudaFuncSetAttribute(k_incoherent, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const bool multi = !(a.gpc == IC_WARPS && a.tt == 1);
+    e = multi ? cudaFuncSetAttribute(k_incoherent<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
+              : cudaFuncSetAttribute(k_incoherent<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    dim3 grid((unsigned)((nt_out + IC_TILE - 1) / IC_TILE), (unsigned)((ngroups + IC_WARPS - 1) / IC_WARPS), (unsigned)g.ndm);
-    k_incoherent<<<grid, 32 * IC_WARPS, smem, st>>>(a);
+    dim3 grid((unsigned)((nt_out + IC_TILE * a.tt - 1) / (IC_TILE * a.tt)), (unsigned)((ngroups + a.gpc - 1) / a.gpc), (unsigned)g.ndm);
+    if (multi) k_incoherent<true><<<grid, 32 * IC_WARPS, smem, st>>>(a);
+    else k_incoherent<false><<<grid, 32 * IC_WARPS, smem, st>>>(a);
     e = cudaGetLastError();
     if (e == cudaSuccess) ++*launches;
     return e;

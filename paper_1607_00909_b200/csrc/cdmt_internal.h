@@ -43,7 +43,7 @@ cudaError_t launch_forward(const Geometry &g, const Workspace &ws, const void *d
 // d_segsum (may be null): block sums [ndm][nblock_total][nch] x (sum I, sum I^2); *sums_done is cleared if the
 // kernel chosen cannot take them (the caller then runs launch_block_sums over the finished filterbank)
 cudaError_t launch_fused(const Geometry &g, const Workspace &ws, const float2 *spec, int unit0,
-                         int nunits, float *d_out, long long out_stride_dm, int dm_tile,
+                         int nunits, float *d_out, long long out_stride_dm, int out_pitch, int dm_tile,
                          int accurate, int force_generic, const double *h_dm, const double *h_fcen,
                          double *d_segsum, int nblock_total, bool *sums_done,
                          cudaStream_t st, long long *launches);
@@ -78,7 +78,7 @@ struct IncoherentTables {            // host side, owned by the plan (must outli
 bool incoherent_plan(const Geometry &g, const double *h_fcen, int nfine, const double *ddm, IncoherentTables *T);
 size_t incoherent_workspace_bytes(const IncoherentTables &T);
 // false if the shift range or the number of trial groups is beyond what the kernel can be launched with
-bool incoherent_config(const IncoherentTables &T, int *cc, int *tw, size_t *smem);
+bool incoherent_config(const IncoherentTables &T, int *cc, int *tw, int *gpc, int *tt, size_t *smem);
 void incoherent_release(IncoherentTables *T);
 cudaError_t launch_incoherent(const Geometry &g, IncoherentTables &T, const float *d_fb, long long fb_stride_dm,
                               long long nt_in, float *d_ts, long long ts_stride_dm, long long ts_pitch,

@@ -238,3 +238,44 @@ def test_suggest_sizes_follow_eq2_and_are_legal(cdmt):
         kw.update(bad)
         with pytest.raises(cdmt.CdmtError):
             cdmt.cdmt_suggest_sizes(**kw)
+
+
+def test_multiplan_partitions_the_band_from_eq2(cdmt):
+    """N4: groups of subbands sized from the dispersion sweep, one common time grid.
+    Host arithmetic only."""
+    # the paper's survey band: 200 subbands from 114.93 MHz (PAPER.md:137, 167), 8 channels, DM <= 79.5
+    fcen = 114.93 + synth.BW_MHZ * (np.arange(200) + 0.5)
+    dm = 0.5 + np.arange(80)
+    mp = cdmt.cdmt_multiplan_create(200, fcen, synth.BW_MHZ, 8, 1, dm, min_efficiency=0.9, max_groups=4)
+    T = 2 ** 20
+    q = cdmt.cdmt_multiplan_query(mp, T)
+    assert 1 < q["ngroups"] <= 4
+    groups = [cdmt.cdmt_multiplan_group(mp, g, T) for g in range(q["ngroups"])]
+    # contiguous cover of the band, sizes that shrink (or stay) with frequency, overlap from Eq. 2 per group
+    assert groups[0]["first_subband"] == 0 and sum(g["nsub"] for g in groups) == 200
+    for a, b in zip(groups, groups[1:]):
+        assert b["first_subband"] == a["first_subband"] + a["nsub"]
+        assert b["nfft"] == a["nfft"] and b["noverlap"] < a["noverlap"]
+    tstart = max(g["noverlap"] // 2 for g in groups)
+    for g in groups:
+        lo = fcen[g["first_subband"]]
+        nfft, nov = cdmt.cdmt_suggest_sizes([lo], synth.BW_MHZ, 8, 1, 79.5, min_efficiency=0.9)
+        assert g["noverlap"] == nov and g["nfft"] >= nfft and g["nfft"] == groups[0]["nfft"]
+        assert g["first_sample"] == tstart - g["noverlap"] // 2          # every group's row 0 starts at tstart
+        step, vd = g["nfft"] - g["noverlap"], (g["nfft"] - g["noverlap"]) // 8
+        assert g["nout"] == ((T - g["first_sample"] - g["nfft"]) // step + 1) * vd
+    assert q["nout_valid"] == min(g["nout"] for g in groups) and q["nout_alloc"] == max(g["nout"] for g in groups)
+    kept = sum(g["nsub"] * (g["nfft"] - g["noverlap"]) / g["nfft"] for g in groups) / 200
+    assert abs(q["kept_fraction"] - kept) < 1e-12
+    # against the paper's one pair for the whole band (N_bin 65536, n_d 2048 x n_c 8: PAPER.md:139): 75 % kept
+    assert q["kept_fraction"] > 0.9 > (65536 - 2048 * 8) / 65536
+    # one group = one plan for the lowest subband's sizes
+    one = cdmt.cdmt_multiplan_create(200, fcen, synth.BW_MHZ, 8, 1, dm, min_efficiency=0.9, max_groups=1)
+    g1 = cdmt.cdmt_multiplan_group(one, 0, T)
+    assert cdmt.cdmt_multiplan_query(one, T)["ngroups"] == 1 and g1["nsub"] == 200 and g1["first_sample"] == 0
+    assert cdmt.cdmt_multiplan_query(one, T)["kept_fraction"] < q["kept_fraction"]
+    with pytest.raises(cdmt.CdmtError):
+        cdmt.cdmt_multiplan_create(3, [120.0, 119.0, 121.0], synth.BW_MHZ, 8, 1, dm)     # not ascending
+    with pytest.raises(cdmt.CdmtError):
+        cdmt.cdmt_multiplan_query(mp, 1000)                                              # shorter than a block
+    cdmt.cdmt_multiplan_destroy(mp)

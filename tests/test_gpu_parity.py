@@ -440,3 +440,47 @@ def test_execute_is_cuda_graph_capturable(cdmt):
     torch.cuda.synchronize()
     want = orc.run(orc.Params(**cfg2.plan_kwargs()), x2)
     check_filterbank(out.cpu().numpy(), want)
+
+
+def test_multiplan_groups_against_the_oracle_on_a_common_time_grid(cdmt):
+    """N4: a multiplan sizes groups of subbands from Eq. 2 and writes ONE filterbank.
+    Each group's columns must equal the oracle run with that group's subbands and sizes on the input from the
+    group's first sample on; an undispersed impulse must land in the same row in every group (common time
+    grid); rows a group does not produce stay untouched."""
+    nsub, nchan, ndec = 12, 8, 8
+    fcen = 114.93 + synth.BW_MHZ * 16 * (np.arange(nsub) + 0.5)          # a wide band: the sweep falls by 5x
+    dm = np.array([0.0, 20.0, 79.5])
+    T = 2 ** 17 + 4096
+    mp = cdmt.cdmt_multiplan_create(nsub, fcen, synth.BW_MHZ, nchan, ndec, dm, min_efficiency=0.9, max_groups=3)
+    q = cdmt.cdmt_multiplan_query(mp, T)
+    assert q["ngroups"] == 3
+    cfg = synth.small_config(nsub=nsub, nsamp=T, nfft=32768, noverlap=4096, nchan=nchan, ndec=ndec, dm=tuple(dm))
+    cfg.fcen_mhz = fcen
+    x = synth.generate(cfg)
+    n0 = 40000
+    x[:, :, n0] += 300.0                                                  # undispersed impulse, every subband
+    d_in = torch.from_numpy(x).cuda()
+    nch = nsub * nchan
+    out = torch.full((len(dm), q["nout_alloc"], nch), float("nan"), dtype=torch.float32, device="cuda")
+    ws = torch.empty(q["workspace_bytes"], dtype=torch.uint8, device="cuda")
+    cdmt.cdmt_multiplan_execute(mp, d_in, T, T, out, q["nout_alloc"] * nch, ws, ws.numel())
+    torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    assert cdmt.cdmt_multiplan_last_launch_count(mp) >= 3 * q["ngroups"]
+    tstart = None
+    for g in range(q["ngroups"]):
+        gi = cdmt.cdmt_multiplan_group(mp, g, T)
+        s0, s1 = gi["first_subband"], gi["first_subband"] + gi["nsub"]
+        p = orc.Params(gi["nsub"], fcen[s0:s1], synth.BW_MHZ, gi["nfft"], gi["noverlap"], nchan, ndec, dm)
+        want = orc.run(p, np.ascontiguousarray(x[s0:s1, :, gi["first_sample"]:]))
+        assert want.shape[1] == gi["nout"]
+        cols = slice((nsub - s1) * nchan, (nsub - s0) * nchan)            # descending frequency
+        check_filterbank(got[:, :gi["nout"], cols], want)
+        assert np.isnan(got[:, gi["nout"]:, cols]).all()                  # nothing written beyond the group's rows
+        t0 = gi["first_sample"] + gi["noverlap"] // 2
+        tstart = t0 if tstart is None else tstart
+        assert t0 == tstart
+        # the impulse: same row in every group at DM 0
+        row = (n0 - tstart) // (nchan * ndec)
+        assert (got[0, :q["nout_valid"], cols].sum(-1).argmax() == row)
+    assert not np.isnan(got[:, :q["nout_valid"]]).any()
