@@ -194,6 +194,70 @@ def run_reference(args, cfg, rank, world):
     print(json.dumps(line), flush=True)
 
 
+def run_survey(args):
+    """--survey: the paper's pilot-survey band (200 subbands of 195.31 kHz from 114.93 MHz,
+    8 channels per subband, 80 DM trials 0.5 ... 79.5) through (a) one plan with the paper's own sizes
+    (N_bin 65536, n_d 2048 channelised samples = 16384 input samples for every subband), (b) a multiplan
+    with one group (overlap from Eq. 2 at the lowest subband) and (c) a multiplan with four groups
+    (sizes that follow the observing frequency).  The paper does not integrate in time; here
+    ndec = 8 keeps the output of 2^20 samples at 8 GB.  One JSON line."""
+    import torch
+    from paper_1607_00909_b200 import cdmt
+    dev = torch.device("cuda", 0)
+    nsub, nchan, ndec, T = 200, 8, 8, 2 ** 20
+    fcen = 114.93 + synth.BW_MHZ * (np.arange(nsub) + 0.5)
+    dm = 0.5 + np.arange(80.0)
+    g = torch.Generator(device=dev)
+    g.manual_seed(5)
+    d_in = torch.view_as_complex(torch.randn((nsub, 2, T, 2), generator=g, device=dev, dtype=torch.float32) * 0.7071)
+    nch = nsub * nchan
+    stream = torch.cuda.current_stream()
+
+    def time_it(fn):
+        for _ in range(max(args.warmup, 3)):
+            fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        for _ in range(args.steps):
+            fn()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / args.steps
+
+    rows = []
+    plan = cdmt.cdmt_plan_create(nsub, fcen, synth.BW_MHZ, 65536, 16384, nchan, ndec, dm)
+    q = cdmt.cdmt_plan_query(plan, T)
+    out = torch.empty((len(dm), q["nout_per_chan"], nch), dtype=torch.float32, device=dev)
+    ws = torch.empty(q["workspace_bytes"], dtype=torch.uint8, device=dev)
+    ms = time_it(lambda: cdmt.cdmt_execute(plan, d_in, T, T, out, out[0].numel(), ws, ws.numel(), stream))
+    rows.append({"what": "one plan, the paper's sizes (nfft 65536, noverlap 16384)", "groups": 1, "kept_fraction": 0.75,
+                 "ms_per_step": ms, "out_samples_per_chan": q["nout_per_chan"],
+                 "output_samples_x_dm_per_s": q["nout_per_chan"] * nch * len(dm) / (ms * 1e-3)})
+    del out, ws
+    for G in (1, 4):
+        mp = cdmt.cdmt_multiplan_create(nsub, fcen, synth.BW_MHZ, nchan, ndec, dm, min_efficiency=0.9, max_groups=G)
+        q = cdmt.cdmt_multiplan_query(mp, T)
+        out = torch.empty((len(dm), q["nout_alloc"], nch), dtype=torch.float32, device=dev)
+        ws = torch.empty(q["workspace_bytes"], dtype=torch.uint8, device=dev)
+        ms = time_it(lambda: cdmt.cdmt_multiplan_execute(mp, d_in, T, T, out, out[0].numel(), ws, ws.numel(), stream))
+        grp = [cdmt.cdmt_multiplan_group(mp, i, T) for i in range(q["ngroups"])]
+        rows.append({"what": "multiplan, max_groups %d (nfft %d; noverlap %s)" % (G, grp[0]["nfft"], [x["noverlap"] for x in grp]),
+                     "groups": q["ngroups"], "kept_fraction": q["kept_fraction"], "ms_per_step": ms,
+                     "out_samples_per_chan": q["nout_valid"],
+                     "output_samples_x_dm_per_s": q["nout_valid"] * nch * len(dm) / (ms * 1e-3)})
+        del out, ws
+    best = rows[-1]
+    line = {"metric": METRIC, "value": float(nsub) * T * len(dm) / (best["ms_per_step"] * 1e-3), "unit": UNIT, "n_gpus": 1,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": best["ms_per_step"],
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "survey band of PAPER.md:137-139: 200 subbands from 114.93 MHz x 2^20 samples, nchan=8 "
+                                   "ndec=8, 80 DM trials 0.5..79.5, complex64 noise in; sizes per group of subbands",
+                       "nsub": nsub, "nsamp": T, "nchan": nchan, "ndec": ndec, "ndm": len(dm)},
+            "real_time_factor": T * synth.TSAMP_S / (best["ms_per_step"] * 1e-3), "variants": rows}
+    print(json.dumps(line), flush=True)
+
+
 def workload_config(cfg, args):
     return {"workload": "%s: %d subbands x 2^%d samples, nfft=%d noverlap=%d nchan=%d ndec=%d, %d DM trials, %s in"
             % (cfg.name, cfg.nsub, int(np.log2(cfg.nsamp)), cfg.nfft, cfg.noverlap, cfg.nchan, cfg.ndec,
@@ -228,7 +292,12 @@ def main():
     ap.add_argument("--no-redigitize", action="store_true", help="skip the extra cdmt_redigitize timing (N1)")
     ap.add_argument("--no-incoherent", action="store_true", help="skip the extra cdmt_incoherent_dedisperse timing (N2)")
     ap.add_argument("--fine-step", type=float, default=0.002, help="fine DM step of the incoherent leg (PAPER.md:141)")
+    ap.add_argument("--survey", action="store_true",
+                    help="N4: the paper's survey band with the paper's sizes against per-group sizes (cdmt_multiplan)")
     args = ap.parse_args()
+    if args.survey:
+        run_survey(args)
+        return
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

@@ -52,7 +52,12 @@ enum {
     CDMT_ERR_ALLOC = 5      /* host allocation failed */
 };
 
-enum { CDMT_IN_CF32 = 0, CDMT_IN_CI8 = 1 };          /* interleaved (re, im) float32 / int8 */
+/* Input layouts.  Interleaved: a row holds complex words (re, im), rows (s, p) = (subband, polarisation).
+ * Planar ("two cufftComplex arrays, one for each polarization" upstream of the unpack step;
+ * telescope back ends write the four real streams Xre, Xim, Yre, Yim separately): a row holds real
+ * words, rows (s, p, part) with part 0 = re, 1 = im.  Row r of subband s starts at element
+ * (rows_per_subband s + r) * in_stride_pol of its word type; in_stride_pol counts words of a row. */
+enum { CDMT_IN_CF32 = 0, CDMT_IN_CI8 = 1, CDMT_IN_PF32 = 2, CDMT_IN_PI8 = 3 };
 enum { CDMT_REF_CHANNEL = 0, CDMT_REF_SUBBAND = 1 }; /* nu_0 of Eq. 1 */
 
 /* Tuning knobs for cdmt_plan_set_option (defaults chosen by the library). */
@@ -118,12 +123,14 @@ int cdmt_plan_query(const cdmt_plan *plan, long long nsamp, int *nblock,
 
 /*
  * Run the whole hot path on device-resident input.
- *   d_in           DEVICE, [nsub][2 pols][..] complex words of the plan's in_dtype, time
- *                  fastest; row (s, p) starts at element (2 s + p) * in_stride_pol.
- *                  Aligned to one complex word (8 bytes float32, 2 bytes int8); 16-byte aligned
- *                  rows let the int8 path use wider loads.
+ *   d_in           DEVICE, [nsub][2 pols][..] complex words (interleaved layouts) or
+ *                  [nsub][2 pols][re, im][..] real words (planar layouts) of the plan's in_dtype, time
+ *                  fastest; consecutive rows are in_stride_pol words apart.  Aligned to one word
+ *                  (8 / 2 / 4 / 1 bytes for CF32 / CI8 / PF32 / PI8); the int8 layouts are read with
+ *                  16-byte loads when the pointer, the row stride, the block step and the pass
+ *                  length are multiples of 16 bytes, else word by word.
  *   nsamp          samples per row to process (>= nfft)
- *   in_stride_pol  distance between consecutive rows, in complex samples (>= nsamp)
+ *   in_stride_pol  distance between consecutive rows, in words of a row (>= nsamp)
  *   d_out          DEVICE float32, DM plane d starts at d * out_stride_dm elements; inside a
  *                  plane [nblock*Vd][nsub*nchan].  Every element of every plane is written.
  *   out_stride_dm  elements between DM planes (>= nblock*Vd*nsub*nchan)
@@ -307,7 +314,8 @@ long long cdmt_min_overlap(const cdmt_plan *plan);
 /* Sizes from the dispersion sweep ("n_d n_c >= r t_d ... for the channel with the lowest
  * frequency"; PAPER.md:175 names the single N_bin / n_d for all subbands as an
  * inefficiency): for the given subbands (call it per subband, or per group of subbands that share a
- * plan) returns the smallest legal noverlap (input samples; a multiple of 2 nchan and of nchan ndec)
+ * plan) returns the smallest noverlap (input samples; a multiple of 2 nchan ndec, so that each discarded edge is a
+ * whole number of integrated samples)
  * that covers the sweep of the lowest channel (REF_CHANNEL) or subband (REF_SUBBAND) at DM
  * dm_max_abs, and the smallest power-of-two nfft this library supports whose kept fraction
  * (nfft - noverlap) / nfft is at least min_efficiency (0 < min_efficiency < 1).  Host arithmetic only.

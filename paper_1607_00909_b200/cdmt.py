@@ -17,7 +17,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("CDMT_LIBRARY") or os.path.join(_HERE, "libcdmt.so")
 
 OK, ERR_ARG, ERR_SIZE, ERR_WORKSPACE, ERR_CUDA, ERR_ALLOC = range(6)
-IN_CF32, IN_CI8 = 0, 1
+IN_CF32, IN_CI8, IN_PF32, IN_PI8 = 0, 1, 2, 3
 REF_CHANNEL, REF_SUBBAND = 0, 1
 OPT_CHUNK_UNITS, OPT_DM_TILE, OPT_ACCURATE_SINCOS, OPT_PROFILE, OPT_FORCE_GENERIC = 0, 1, 2, 3, 4
 OPT_HOST_GROUP_BLOCKS = 5
@@ -407,7 +407,7 @@ def cdmt_measure_fp32_peak(d_scratch, scratch_bytes: int, iters: int = 5, stream
 # Convenience for tests and bench: allocate with torch, call the ABI, return the tensor.
 # ---------------------------------------------------------------------------------------
 def run_on_device(plan: Plan, d_in, nsamp: int, stream=None, out=None, workspace=None):
-    """d_in: CUDA tensor [nsub][2][T] complex64 (or [nsub][2][T][2] int8). Returns
+    """d_in: CUDA tensor [nsub][2][T] complex64, [nsub][2][T][2] int8, or planar [nsub][2][2][T] float32 / int8. Returns
     out [ndm][nblock*Vd][nsub*nchan] float32 (CUDA)."""
     import torch
     q = cdmt_plan_query(plan, nsamp)
@@ -417,6 +417,9 @@ def run_on_device(plan: Plan, d_in, nsamp: int, stream=None, out=None, workspace
         out = torch.empty((plan.ndm, nt, nch), dtype=torch.float32, device=d_in.device)
     if workspace is None:
         workspace = torch.empty(q["workspace_bytes"], dtype=torch.uint8, device=d_in.device)
-    stride_pol = d_in.stride(1) // (2 if plan.in_dtype == IN_CI8 else 1)
+    if plan.in_dtype in (IN_PF32, IN_PI8):
+        stride_pol = d_in.stride(2)          # [nsub][2][2 parts][T] real words
+    else:
+        stride_pol = d_in.stride(1) // (2 if plan.in_dtype == IN_CI8 else 1)
     cdmt_execute(plan, d_in, nsamp, stride_pol, out, nt * nch, workspace, workspace.numel(), stream)
     return out

@@ -105,7 +105,7 @@ extern "C" int cdmt_plan_create(cdmt_plan **plan, int nsub, const double *fcen_m
     *plan = nullptr;
     if (!fcen_mhz || !dm || nsub < 1 || ndm < 1) return CDMT_ERR_ARG;
     if (!(bw_mhz > 0.0) || !std::isfinite(bw_mhz)) return CDMT_ERR_ARG;
-    if (in_dtype != CDMT_IN_CF32 && in_dtype != CDMT_IN_CI8) return CDMT_ERR_ARG;
+    if (in_dtype < CDMT_IN_CF32 || in_dtype > CDMT_IN_PI8) return CDMT_ERR_ARG;
     if (chirp_ref != CDMT_REF_CHANNEL && chirp_ref != CDMT_REF_SUBBAND) return CDMT_ERR_ARG;
     for (int s = 0; s < nsub; ++s)
         if (!std::isfinite(fcen_mhz[s]) || !(fcen_mhz[s] - 0.5 * bw_mhz > 0.0)) return CDMT_ERR_ARG;
@@ -278,7 +278,7 @@ static int validate_input(const cdmt_plan *plan, const void *d_in, long long nsa
     const Geometry &g = plan->g;
     // one complex word: the forward pass reads 8-byte (float32) or 2-byte (int8) words and takes wider
     // loads only where the address allows; cdmt_unpack's float4 path wants 16 bytes (align16)
-    const uintptr_t word = g.in_dtype == CDMT_IN_CF32 ? (align16 ? 16 : 8) : 2;
+    const uintptr_t word = g.in_dtype == CDMT_IN_CF32 ? (align16 ? 16 : 8) : (uintptr_t)in_word_bytes(g.in_dtype);
     if ((reinterpret_cast<uintptr_t>(d_in) & (word - 1)) != 0) return CDMT_ERR_ARG;
     if (nsamp < g.nfft) return CDMT_ERR_SIZE;
     if (in_stride_pol < nsamp) return CDMT_ERR_SIZE;
@@ -471,15 +471,15 @@ static int host_layout(const cdmt_plan *plan, long long nsamp, int out_kind, Hos
     const long long nb = nblock_for(g, nsamp);
     if (nb < 1) return CDMT_ERR_SIZE;
     if (out_kind != CDMT_OUT_F32 && out_kind != CDMT_OUT_U8) return CDMT_ERR_ARG;
-    const long long esz = g.in_dtype == CDMT_IN_CI8 ? 2 : 8;
+    const long long esz = in_word_bytes(g.in_dtype), rps = in_rows_per_sub(g.in_dtype);
     L->gb = host_group_blocks(plan, nb);
     L->ngroup = (nb + L->gb - 1) / L->gb;
     long long rowlen = (L->gb - 1) * g.step + g.nfft;
-    rowlen = (rowlen + 7) & ~7LL;  // keep rows 16-byte aligned for both word sizes
+    rowlen = (rowlen + 15) & ~15LL;  // keep rows 16-byte aligned for every word size
     L->in_rowlen = rowlen;
     auto al = [](size_t x) { return (x + 255) & ~(size_t)255; };
     const int nbuf = L->gb < nb ? 2 : 1;  // a single group needs no second buffer
-    L->in_bytes = al((size_t)rowlen * esz * 2 * g.nsub);
+    L->in_bytes = al((size_t)rowlen * esz * rps * g.nsub);
     L->in_off[0] = 0;
     L->in_off[1] = nbuf == 2 ? L->in_bytes : 0;
     L->ws_off = L->in_bytes * nbuf;
@@ -518,11 +518,11 @@ extern "C" int cdmt_host_layout(const cdmt_plan *plan, long long nsamp, int out_
     if (rc) return rc;
     const Geometry &g = plan->g;
     const long long nb = nblock_for(g, nsamp);
-    const size_t esz = g.in_dtype == CDMT_IN_CI8 ? 2 : 8;
+    const size_t esz = (size_t)in_word_bytes(g.in_dtype), rps = (size_t)in_rows_per_sub(g.in_dtype);
     size_t in = 0;
     for (long long b0 = 0; b0 < nb; b0 += L.gb) {
         const long long nbg = (nb - b0 < L.gb) ? nb - b0 : L.gb;
-        in += (size_t)((nbg - 1) * g.step + g.nfft) * esz * 2 * g.nsub;
+        in += (size_t)((nbg - 1) * g.step + g.nfft) * esz * rps * g.nsub;
     }
     const size_t samples = (size_t)g.ndm * (size_t)(nb * g.vdec) * (size_t)g.nsub * g.nchan;
     if (scratch_bytes) *scratch_bytes = L.total;
@@ -580,7 +580,7 @@ extern "C" int cdmt_execute_host_async(cdmt_plan *plan, const void *h_in, long l
     if (!plan_host_pipeline(plan)) return check_cuda(cudaErrorUnknown);
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const long long nb = nblock_for(g, nsamp);
-    const long long esz = g.in_dtype == CDMT_IN_CI8 ? 2 : 8;
+    const long long esz = in_word_bytes(g.in_dtype), rps = in_rows_per_sub(g.in_dtype);
     char *base = reinterpret_cast<char *>(d_scratch);
     const size_t nchtot = (size_t)g.nsub * g.nchan;
     const size_t plane_host = (size_t)nb * g.vdec * nchtot;
@@ -610,7 +610,7 @@ extern "C" int cdmt_execute_host_async(cdmt_plan *plan, const void *h_in, long l
         }
         int r = check_cuda(copy_rows_async(base + L.in_off[k], (size_t)L.in_rowlen * esz,
                                            reinterpret_cast<const char *>(h_in) + (size_t)b0 * g.step * esz,
-                                           (size_t)in_stride_pol * esz, (size_t)len * esz, (size_t)2 * g.nsub,
+                                           (size_t)in_stride_pol * esz, (size_t)len * esz, (size_t)rps * g.nsub,
                                            cudaMemcpyHostToDevice, plan->s_in));
         if (r) return r;
         return check_cuda(cudaEventRecord(plan->ev_h2d[k], plan->s_in));
@@ -884,11 +884,9 @@ extern "C" int cdmt_suggest_sizes(int nsub, const double *fcen_mhz, double bw_mh
         td = cdmt_sweep_seconds(fmin, bw_mhz, dm_max_abs);
     }
     const long long sweep = (long long)std::ceil(td * bw_mhz * 1e6);   // input samples (r t_d)
-    // noverlap: multiple of 2 nchan (half per edge, whole channelised samples) and of nchan ndec
-    long long q = 2LL * nchan, r = (long long)nchan * ndec;
-    long long a = q, b = r;
-    while (b) { const long long t = a % b; a = b; b = t; }
-    const long long unit = q / a * r;
+    // noverlap: a multiple of 2 nchan ndec -- half per edge, and each half a whole number of INTEGRATED
+    // samples (what the packed fused kernels need; it also satisfies the plan's two divisibility rules)
+    const long long unit = 2LL * nchan * ndec, r = (long long)nchan * ndec;
     const long long ov = (sweep + unit - 1) / unit * unit;
     // nfft: smallest power of two whose kept fraction reaches min_efficiency and that the kernels support
     for (long long n = 256; n <= (1LL << 20); n <<= 1) {
@@ -1084,7 +1082,7 @@ extern "C" int cdmt_multiplan_execute(cdmt_multiplan *mp, const void *d_in, long
     if (!mp || !d_in || !d_out || !d_workspace) return CDMT_ERR_ARG;
     if ((reinterpret_cast<uintptr_t>(d_workspace) & 255) != 0 || (reinterpret_cast<uintptr_t>(d_out) & 3) != 0)
         return CDMT_ERR_ARG;
-    const uintptr_t word = mp->in_dtype == CDMT_IN_CI8 ? 2 : 8;
+    const uintptr_t word = (uintptr_t)in_word_bytes(mp->in_dtype), rps = (uintptr_t)in_rows_per_sub(mp->in_dtype);
     if ((reinterpret_cast<uintptr_t>(d_in) & (word - 1)) != 0) return CDMT_ERR_ARG;
     if (in_stride_pol < nsamp) return CDMT_ERR_SIZE;
     MultiSizes z;
@@ -1096,7 +1094,7 @@ extern "C" int cdmt_multiplan_execute(cdmt_multiplan *mp, const void *d_in, long
     mp->last_launches = 0;
     for (size_t i = 0; i < mp->plans.size(); ++i) {
         cdmt_plan *p = mp->plans[i];
-        const char *in = static_cast<const char *>(d_in) + ((size_t)2 * mp->sub0[i] * (size_t)in_stride_pol + (size_t)z.delta[i]) * word;
+        const char *in = static_cast<const char *>(d_in) + ((size_t)rps * mp->sub0[i] * (size_t)in_stride_pol + (size_t)z.delta[i]) * word;
         // descending frequency: the highest group comes first in a row
         float *out = d_out + (size_t)(mp->nsub - mp->sub0[i] - mp->nsubg[i]) * mp->nchan;
         rc = run_chunks(p, in, in_stride_pol, z.nblock[i], out, out_stride_dm, nullptr, d_workspace, workspace_bytes,

@@ -18,6 +18,11 @@ struct Geometry {
     int lo_bits;
 };
 
+// input layouts (CDMT_IN_*): bytes of one word of a row and rows per subband
+// 0 interleaved float32 (8, 2), 1 interleaved int8 (2, 2), 2 planar float32 (4, 4), 3 planar int8 (1, 4)
+inline int in_word_bytes(int in_dtype) { return in_dtype == 0 ? 8 : in_dtype == 1 ? 2 : in_dtype == 2 ? 4 : 1; }
+inline int in_rows_per_sub(int in_dtype) { return in_dtype >= 2 ? 4 : 2; }
+
 // Device pointers into the workspace (all 256-byte aligned).
 struct Workspace {
     double *dm;         // [ndm]

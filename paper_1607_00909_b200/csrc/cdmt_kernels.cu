@@ -95,18 +95,55 @@ k_init_tables(const InitArgs a, const __grid_constant__ DoubleChunk dm, const __
 // ------------------------------------------------------------------------------------
 // input words -> complex float (Alg. 1 l.95 "unpack")
 // ------------------------------------------------------------------------------------
+// Input layouts (include/cdmt.h CDMT_IN_*): 0 interleaved float32, 1 interleaved int8, 2 planar float32,
+// 3 planar int8.  Interleaved: row (s, p) = complex words; planar: rows (s, p, re) and (s, p, im) of real
+// words, `stride` apart ("unpacked into two cufftComplex arrays, one for each polarization").
 template <int IN>
-__device__ __forceinline__ float2 load_sample(const void *base, size_t idx);
+struct InWord;
+template <> struct InWord<0> { static constexpr int bytes = 8, rows = 2; };
+template <> struct InWord<1> { static constexpr int bytes = 2, rows = 2; };
+template <> struct InWord<2> { static constexpr int bytes = 4, rows = 4; };
+template <> struct InWord<3> { static constexpr int bytes = 1, rows = 4; };
+
+// first word of polarisation p of subband s (planar: of its real part)
+template <int IN>
+__device__ __forceinline__ size_t in_row0(int s, int p, long long stride)
+{
+    return (size_t)(InWord<IN>::rows * s + (InWord<IN>::rows / 2) * p) * (size_t)stride;
+}
+
+template <int IN>
+__device__ __forceinline__ float2 load_sample(const void *base, size_t idx, long long stride);
 template <>
-__device__ __forceinline__ float2 load_sample<0>(const void *base, size_t idx)
+__device__ __forceinline__ float2 load_sample<0>(const void *base, size_t idx, long long)
 {
     return __ldg(reinterpret_cast<const float2 *>(base) + idx);
 }
 template <>
-__device__ __forceinline__ float2 load_sample<1>(const void *base, size_t idx)
+__device__ __forceinline__ float2 load_sample<1>(const void *base, size_t idx, long long)
 {
     char2 q = __ldg(reinterpret_cast<const char2 *>(base) + idx);
     return make_float2((float)q.x, (float)q.y);
+}
+template <>
+__device__ __forceinline__ float2 load_sample<2>(const void *base, size_t idx, long long stride)
+{
+    const float *f = reinterpret_cast<const float *>(base) + idx;
+    return make_float2(__ldg(f), __ldg(f + stride));
+}
+template <>
+__device__ __forceinline__ float2 load_sample<3>(const void *base, size_t idx, long long stride)
+{
+    const signed char *f = reinterpret_cast<const signed char *>(base) + idx;
+    return make_float2((float)__ldg(f), (float)__ldg(f + stride));
+}
+
+__device__ __forceinline__ void unpack_int8x4(unsigned w, float (&f)[4])
+{
+    f[0] = (float)(signed char)(w & 0xff);
+    f[1] = (float)(signed char)((w >> 8) & 0xff);
+    f[2] = (float)(signed char)((w >> 16) & 0xff);
+    f[3] = (float)(signed char)(w >> 24);
 }
 
 // blocks[(b nsub + s)][p][n] = in[s][p][b step + n]; 4 samples per thread
@@ -116,7 +153,7 @@ __global__ void __launch_bounds__(256) k_unpack(const void *__restrict__ in, lon
 {
     const int row = blockIdx.x;  // (b nsub + s) * 2 + p
     const int unit = row >> 1, p = row & 1, b = unit / nsub, s = unit % nsub;
-    const size_t src0 = (size_t)(2 * s + p) * (size_t)in_stride_pol + (size_t)b * step;
+    const size_t src0 = in_row0<IN>(s, p, in_stride_pol) + (size_t)b * step;
     float2 *dst = blocks + (size_t)row * nfft;
     const int n0 = (blockIdx.y * 256 + threadIdx.x) * 4;
     if (n0 >= nfft) return;
@@ -126,13 +163,9 @@ __global__ void __launch_bounds__(256) k_unpack(const void *__restrict__ in, lon
         reinterpret_cast<float4 *>(dst + n0)[0] = a;
         reinterpret_cast<float4 *>(dst + n0)[1] = c;
     } else {
-        const char2 *src = reinterpret_cast<const char2 *>(in) + src0 + n0;
         float2 v[4];
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            char2 q = __ldg(src + i);
-            v[i] = make_float2((float)q.x, (float)q.y);
-        }
+        for (int i = 0; i < 4; ++i) v[i] = load_sample<IN>(in, src0 + n0 + i, in_stride_pol);
         reinterpret_cast<float4 *>(dst + n0)[0] = make_float4(v[0].x, v[0].y, v[1].x, v[1].y);
         reinterpret_cast<float4 *>(dst + n0)[1] = make_float4(v[2].x, v[2].y, v[3].x, v[3].y);
     }
@@ -152,7 +185,8 @@ template <int L, int MODE, int IN>
 __global__ void __launch_bounds__(L) k_fwd_pass(const void *__restrict__ src_v, float2 *__restrict__ dst,
                                                 const float2 *__restrict__ tw, const float2 *__restrict__ tw_lo,
                                                 const float2 *__restrict__ tw_hi, int lo_bits, int nfft, int n1,
-                                                int n2, int nsub, int step, long long in_stride_pol, int unit0)
+                                                int n2, int nsub, int step, long long in_stride_pol, int unit0,
+                                                int vec16)
 {
     constexpr int NT = L;
     using Plan = RadixPlan<L>;
@@ -167,11 +201,45 @@ __global__ void __launch_bounds__(L) k_fwd_pass(const void *__restrict__ src_v, 
 
     if (MODE == 0) {
         const int unit = unit0 + (row >> 1), b = unit / nsub, s = unit % nsub;
-        const size_t src0 = (size_t)(2 * s + p) * (size_t)in_stride_pol + (size_t)b * step + (size_t)tile * FWD_BATCH;
+        const size_t src0 = in_row0<IN>(s, p, in_stride_pol) + (size_t)b * step + (size_t)tile * FWD_BATCH;
+        if ((IN == 1 || IN == 3) && vec16) {
+            // int8, 16-byte loads along time: one row of the tile (16 samples) is 32 interleaved bytes = two
+            // loads, or 16 + 16 planar bytes = one load per part.  vec16: every such address is 16-byte aligned.
+            constexpr int PER_ROW = IN == 1 ? 2 : 1;
+#pragma unroll 4
+            for (int e = tid; e < L * PER_ROW; e += NT) {
+                const int n1i = e / PER_ROW, half = e % PER_ROW;
+                const signed char *q = reinterpret_cast<const signed char *>(src_v) +
+                                       (src0 + (size_t)n1i * n2) * InWord<IN>::bytes + 16 * half;
+                const uint4 w = __ldg(reinterpret_cast<const uint4 *>(q));
+                const unsigned ww[4] = {w.x, w.y, w.z, w.w};
+                if (IN == 1) {
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        float f[4];
+                        unpack_int8x4(ww[k], f);
+                        smem[Addr::at(n1i, 8 * half + 2 * k)] = make_float2(f[0], f[1]);
+                        smem[Addr::at(n1i, 8 * half + 2 * k + 1)] = make_float2(f[2], f[3]);
+                    }
+                } else {
+                    const uint4 wi = __ldg(reinterpret_cast<const uint4 *>(q + in_stride_pol));
+                    const unsigned wwi[4] = {wi.x, wi.y, wi.z, wi.w};
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        float fr[4], fi[4];
+                        unpack_int8x4(ww[k], fr);
+                        unpack_int8x4(wwi[k], fi);
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) smem[Addr::at(n1i, 4 * k + j)] = make_float2(fr[j], fi[j]);
+                    }
+                }
+            }
+        } else {
 #pragma unroll 16  // all 16 loads of a thread in flight (HBM latency; measured 11.8 -> 9.6 ms per c3 step)
-        for (int e = tid; e < L * FWD_BATCH; e += NT) {
-            const int n1i = e / FWD_BATCH, col = e % FWD_BATCH;
-            smem[Addr::at(n1i, col)] = load_sample<IN>(src_v, src0 + (size_t)n1i * n2 + col);
+            for (int e = tid; e < L * FWD_BATCH; e += NT) {
+                const int n1i = e / FWD_BATCH, col = e % FWD_BATCH;
+                smem[Addr::at(n1i, col)] = load_sample<IN>(src_v, src0 + (size_t)n1i * n2 + col, in_stride_pol);
+            }
         }
     } else {
         const float2 *src = reinterpret_cast<const float2 *>(src_v) + plane + (size_t)tile * FWD_BATCH * n2;
@@ -304,10 +372,12 @@ cudaError_t launch_unpack(const Geometry &g, const void *d_in, long long in_stri
                           float2 *d_blocks, cudaStream_t st, long long *launches)
 {
     dim3 grid((unsigned)(nblock * g.nsub * 2), (unsigned)((g.nfft / 4 + 255) / 256));
-    if (g.in_dtype == 0)
-        k_unpack<0><<<grid, 256, 0, st>>>(d_in, in_stride_pol, g.nsub, g.nfft, g.step, d_blocks);
-    else
-        k_unpack<1><<<grid, 256, 0, st>>>(d_in, in_stride_pol, g.nsub, g.nfft, g.step, d_blocks);
+    switch (g.in_dtype) {
+    case 0: k_unpack<0><<<grid, 256, 0, st>>>(d_in, in_stride_pol, g.nsub, g.nfft, g.step, d_blocks); break;
+    case 1: k_unpack<1><<<grid, 256, 0, st>>>(d_in, in_stride_pol, g.nsub, g.nfft, g.step, d_blocks); break;
+    case 2: k_unpack<2><<<grid, 256, 0, st>>>(d_in, in_stride_pol, g.nsub, g.nfft, g.step, d_blocks); break;
+    default: k_unpack<3><<<grid, 256, 0, st>>>(d_in, in_stride_pol, g.nsub, g.nfft, g.step, d_blocks); break;
+    }
     ++*launches;
     return cudaGetLastError();
 }
@@ -325,11 +395,20 @@ static cudaError_t launch_fwd_L(int mode, const Geometry &g, const Workspace &ws
         e = cudaFuncSetAttribute(k_fwd_pass<L, MODE, IN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
         if (e != cudaSuccess) return e;                                                                            \
         k_fwd_pass<L, MODE, IN><<<grid, L, smem, st>>>(src, dst, tw, ws.tw4_lo, ws.tw4_hi, g.lo_bits, g.nfft,      \
-                                                       g.n1, g.n2, g.nsub, g.step, in_stride_pol, unit0);         \
+                                                       g.n1, g.n2, g.nsub, g.step, in_stride_pol, unit0, vec16);  \
     } while (0)
+    // int8 input: 16-byte loads along time where every tile row starts on a 16-byte boundary
+    const int wb = g.in_dtype == 1 ? 2 : 1;
+    const int vec16 = (g.in_dtype == 1 || g.in_dtype == 3) && (reinterpret_cast<uintptr_t>(src) & 15) == 0 &&
+                      ((long long)in_stride_pol * wb) % 16 == 0 && ((long long)g.step * wb) % 16 == 0 &&
+                      ((long long)g.n2 * wb) % 16 == 0;
     if (mode == 0) {
-        if (g.in_dtype == 0) CDMT_FWD(0, 0);
-        else CDMT_FWD(0, 1);
+        switch (g.in_dtype) {
+        case 0: CDMT_FWD(0, 0); break;
+        case 1: CDMT_FWD(0, 1); break;
+        case 2: CDMT_FWD(0, 2); break;
+        default: CDMT_FWD(0, 3); break;
+        }
     } else {
         CDMT_FWD(1, 0);
     }

@@ -484,3 +484,72 @@ def test_multiplan_groups_against_the_oracle_on_a_common_time_grid(cdmt):
         row = (n0 - tstart) // (nchan * ndec)
         assert (got[0, :q["nout_valid"], cols].sum(-1).argmax() == row)
     assert not np.isnan(got[:, :q["nout_valid"]]).any()
+
+
+# ---------------------------------------------------------------- N3: planar input layouts
+def planar_of(x, in_dtype):
+    """[nsub][2][T] complex64 or [nsub][2][T][2] int8 (interleaved) -> [nsub][2][2 parts][T] real words."""
+    if in_dtype == synth.IN_CI8:
+        return np.ascontiguousarray(np.moveaxis(x, 3, 2))
+    return np.ascontiguousarray(np.stack([x.real, x.imag], axis=2).astype(np.float32))
+
+
+@pytest.mark.parametrize("in_dtype", [synth.IN_CF32, synth.IN_CI8])
+def test_planar_input_unpack_and_parity(cdmt, in_dtype):
+    """CDMT_IN_PF32 / CDMT_IN_PI8 ([S][Xre, Xim, Yre, Yim][T]): cdmt_unpack is bit exact,
+    the whole path matches the oracle (which is fed the same samples interleaved) and is bit for bit the
+    interleaved plan's output; also through the host path, and with a row stride that defeats the 16-byte
+    loads of the int8 path."""
+    cfg = synth.small_config(nsub=3, nsamp=2 ** 15 + 300, nfft=8192, noverlap=2048, nchan=8, ndec=4,
+                             dm=(0.0, 7.5, 30.0), in_dtype=in_dtype)
+    x = synth.generate(cfg)
+    xp = planar_of(x, in_dtype)
+    kw = cfg.plan_kwargs()
+    want = orc.run(orc.Params(**kw), x)
+    base, _ = gpu_run(cdmt, cfg, x)
+    kw["in_dtype"] = cdmt.IN_PI8 if in_dtype == synth.IN_CI8 else cdmt.IN_PF32
+    plan = cdmt.cdmt_plan_create(**kw)
+    T = cfg.nsamp
+    # unpack: bit exact
+    d_in = torch.from_numpy(xp).cuda()
+    B = cfg.nblock
+    blocks = torch.zeros((B * cfg.nsub, 2, cfg.nfft), dtype=torch.complex64, device="cuda")
+    cdmt.cdmt_unpack(plan, d_in, T, T, blocks)
+    torch.cuda.synchronize()
+    xc = x if in_dtype == synth.IN_CF32 else (x[..., 0].astype(np.float32) + 1j * x[..., 1].astype(np.float32))
+    got = blocks.cpu().numpy()
+    for b in range(B):
+        for s in range(cfg.nsub):
+            assert np.array_equal(got[b * cfg.nsub + s], xc[s, :, b * cfg.step:b * cfg.step + cfg.nfft].astype(np.complex64))
+    # whole path, rows T words apart (T % 16 != 0: the int8 path reads word by word) and padded to 16 bytes
+    for stride in (T, (T + 63) // 64 * 64):
+        buf = torch.zeros((cfg.nsub, 2, 2, stride), dtype=d_in.dtype, device="cuda")
+        buf[..., :T] = d_in
+        out = cdmt.run_on_device(plan, buf, T)
+        torch.cuda.synchronize()
+        check_filterbank(out.cpu().numpy(), want)
+        assert np.array_equal(out.cpu().numpy(), base), stride
+    # host path
+    h_in = torch.from_numpy(xp).pin_memory()
+    h_out = torch.empty(base.shape, dtype=torch.float32).pin_memory()
+    cdmt.cdmt_plan_set_option(plan, cdmt.OPT_HOST_GROUP_BLOCKS, 2)
+    nbytes = cdmt.cdmt_host_scratch_bytes(plan, T)
+    scratch = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    cdmt.cdmt_execute_host(plan, h_in.data_ptr(), T, T, h_out.data_ptr(), scratch, nbytes)
+    assert np.array_equal(h_out.numpy(), base)
+
+
+def test_int8_wide_loads_equal_word_loads(cdmt):
+    """The interleaved int8 path takes 16-byte loads when rows are 16-byte aligned: same bits as word loads."""
+    cfg = synth.small_config(nsub=2, nsamp=2 ** 16, nfft=16384, noverlap=4096, nchan=8, ndec=8,
+                             dm=(0.0, 12.0), in_dtype=synth.IN_CI8)
+    x = synth.generate(cfg)
+    plan = cdmt.cdmt_plan_create(**cfg.plan_kwargs())
+    T = cfg.nsamp
+    aligned = torch.from_numpy(x).cuda()                                    # rows 2 T bytes apart: 16-byte aligned
+    a = cdmt.run_on_device(plan, aligned, T).cpu().numpy()
+    buf = torch.zeros((cfg.nsub, 2, T + 3, 2), dtype=torch.int8, device="cuda")   # stride T + 3 words: misaligned rows
+    buf[:, :, :T] = aligned
+    b = cdmt.run_on_device(plan, buf, T).cpu().numpy()
+    assert np.array_equal(a, b)
+    check_filterbank(a, orc.run(orc.Params(**cfg.plan_kwargs()), x))
