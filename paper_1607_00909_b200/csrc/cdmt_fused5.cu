@@ -49,13 +49,9 @@ struct WS {
     static constexpr int IROW = 34;        // float2 per integration row: 32 lanes + 16 bytes
     static constexpr int INTEG = 16 * IROW;
     static constexpr int COL_XA = 0, COL_TW1 = 256, COL_TW2 = 288, COL_TWF = 320, COL_H = 384;
-    static constexpr int NBAR = 8 + 16;    // per group A0 A1 F0 F1; per quadrant full[2] empty[2]
-    static constexpr size_t group_bytes = sizeof(float4) * 2 * EX + sizeof(float2) * NWARP * INTEG;
-    // block sums (SUMS): the FFT lanes hand the two values they stored to the chirp warps through
-    // fsum[slot][group][thread] (float4, four trials deep); the chirp warps leave their pairs in psum[parity][group][q]
-    static constexpr int SUM_SLOTS = 4;
-    static constexpr size_t smem_bytes = 2 * group_bytes + sizeof(uint64_t) * NBAR + 16 +
-                                         sizeof(float4) * SUM_SLOTS * NGRP * NT + sizeof(double2) * 2 * NGRP * NWARP;
+    static constexpr int NBAR = 8 + 16 + 32;  // per group A0 A1 F0 F1; per quadrant H full[2] empty[2]; per (group, quadrant) tile full[2] empty[2]
+    static constexpr size_t group_bytes = sizeof(float4) * 2 * EX + sizeof(float2) * 2 * NWARP * INTEG;  // two tiles per warp
+    static constexpr size_t smem_bytes = 2 * group_bytes + sizeof(uint64_t) * NBAR + 16 + sizeof(double2) * 2 * NGRP * NWARP;
     static constexpr int REGS_FFT = 200, REGS_CHIRP = 104;  // 2 x 200 + 104 = 3 x 168: what the CTA holds at launch
 };
 
@@ -94,8 +90,7 @@ k_fused_ws(const FusedArgs a, const __grid_constant__ DmParams dmp)
     extern __shared__ float4 smem4[];
     uint64_t *bars = reinterpret_cast<uint64_t *>(reinterpret_cast<char *>(smem4) + 2 * G::group_bytes);
     uint32_t *tslot = reinterpret_cast<uint32_t *>(bars + G::NBAR);
-    float4 *fsum = reinterpret_cast<float4 *>(tslot + 4);                                      // [slot][group][NT]
-    double2 *psum = reinterpret_cast<double2 *>(fsum + G::SUM_SLOTS * G::NGRP * NT);             // [parity][group][q]
+    double2 *psum = reinterpret_cast<double2 *>(tslot + 4);   // [parity][group][q]: the chirp warps' (sum I, sum I^2)
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int role = warp >> 2;          // 0, 1: FFT group A, B; NGRP: chirp warps
@@ -115,6 +110,7 @@ k_fused_ws(const FusedArgs a, const __grid_constant__ DmParams dmp)
             for (int k = 0; k < 4; ++k) mbar_init(bars + 4 * g + k, NT);
         for (int k = 0; k < 8; ++k) mbar_init(bars + 8 + k, 1);                       // full[q][buf]: the chirp warp
         for (int k = 0; k < 8; ++k) mbar_init(bars + 16 + k, has_b ? 2 : 1);          // empty[q][buf]: the consumers
+        for (int k = 0; k < 32; ++k) mbar_init(bars + 24 + k, 1);                     // tile full / empty[g][q][buf]
     }
     tmem_fence_before_sync();
     __syncthreads();
@@ -122,6 +118,7 @@ k_fused_ws(const FusedArgs a, const __grid_constant__ DmParams dmp)
     const uint32_t tbase = *tslot;
     const uint32_t tcol = tbase + ((uint32_t)(32 * q) << 16);
     uint64_t *full = bars + 8 + 2 * q, *empty = bars + 16 + 2 * q;
+    // tile hand-over between FFT warp (g, q) and chirp warp q: bars[24 + 4 (4 g + q) + 2 buf] = full, + 1 = empty
 
     const int j1 = t & 15, j2 = t >> 4;      // pass-0 role; pass 1: (j2, t0 = t & 15)
     const int rest = j1 * R2 + j2;           // half-transform input index j = j0 L/16 + rest
@@ -191,33 +188,78 @@ k_fused_ws(const FusedArgs a, const __grid_constant__ DmParams dmp)
         tmem_fence_before_sync();
         __syncthreads();  // X and twiddles are in TMEM
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(G::REGS_CHIRP));
-        // Block sums of trial index j (Alg. 1 l.104): this warp adds, in fp64, the values the FFT lanes of its
-        // quadrant stored (sum and sum of squares), the four chirp warps meet at a named barrier, and two
-        // threads add the four pairs in quadrant order and write them out.
+        // Epilogue of trial index j, for both FFT groups: the FFT warp (g, q) left the 32 powers of each of its
+        // lanes (times t + NT n [+ L]) in a tile; here one lane sums the D adjacent samples of a row (time
+        // integration, north_star), scales and stores them time-major, and -- SUMS -- the warp
+        // adds the stored values and their squares in fp64 (block sums of Alg. 1 l.104), the four chirp warps
+        // meet at a named barrier and one thread per group adds the four pairs in quadrant order.
         const int nchan_total = a.nsub * a.nchan;
         const int ochan = nchan_total - 1 - (s * a.nchan + c);
-        auto block_sums = [&](unsigned j) {
-            double2 *ps = psum + (size_t)(j & 1u) * G::NGRP * G::NWARP;
+        const int il = lane & (DG - 1), g0 = lane - il;
+        const int tgrp = (D > 16) ? (t & ~31) : (t - il);  // first sample of a lane's group, before + NT n
+        auto epilogue = [&](unsigned j) {
+            const unsigned tb = j & 1u, tpar = (j >> 1) & 1u;
+            double2 *ps = psum + (size_t)tb * G::NGRP * G::NWARP;
 #pragma unroll
             for (int g = 0; g < G::NGRP; ++g) {
                 if (g == 1 && !has_b) break;
-                const float4 v = fsum[((size_t)(j & (G::SUM_SLOTS - 1)) * G::NGRP + g) * NT + t];
-                double a1 = ((double)v.x + (double)v.y) + ((double)v.z + (double)v.w);
-                double a2 = fma((double)v.x, (double)v.x, fma((double)v.y, (double)v.y,
-                                fma((double)v.z, (double)v.z, (double)v.w * (double)v.w)));
-                warp_sum_pair(a1, a2);
-                if (lane == 0) ps[g * G::NWARP + q] = make_double2(a1, a2);
-            }
-            asm volatile("bar.sync 1, 128;" ::: "memory");
-            if (t < G::NGRP && (t == 0 || has_b)) {
-                double a1 = 0.0, a2 = 0.0;
+                uint64_t *tbar = bars + 24 + 4 * (4 * g + q) + 2 * tb;
+                const float2 *ib = reinterpret_cast<const float2 *>(smem4 + (size_t)g * (G::group_bytes / sizeof(float4)) + 2 * G::EX) +
+                                   (size_t)(2 * q + tb) * G::INTEG;
+                const int b = a.unit0 / a.nsub + 2 * bp + g;
+                float *outd = a.out + (size_t)(d_begin + (int)j) * (size_t)a.out_stride_dm + (size_t)b * a.vdec * a.out_pitch + ochan;
+                mbar_wait(tbar, tpar);  // the FFT warp has filled the tile
+                double sum1 = 0.0, sum2 = 0.0;
 #pragma unroll
-                for (int w = 0; w < G::NWARP; ++w) {
-                    a1 += ps[t * G::NWARP + w].x;
-                    a2 += ps[t * G::NWARP + w].y;
+                for (int kk = 0; kk < 16 / DG; ++kk) {
+                    const int n = il + DG * kk;
+                    const float4 *row = reinterpret_cast<const float4 *>(ib + n * G::IROW + g0);
+                    P2 acc = pk(0.f, 0.f);
+#pragma unroll
+                    for (int qq = 0; qq < DG / 2; ++qq) {
+                        const float4 f = row[qq];
+                        acc = add2(acc, add2(pk(f.x, f.y), pk(f.z, f.w)));
+                    }
+                    float s0, s1;
+                    upk(acc, s0, s1);
+                    if (D > 16) {
+                        s0 += __shfl_xor_sync(0xffffffffu, s0, 16);
+                        s1 += __shfl_xor_sync(0xffffffffu, s1, 16);
+                    }
+                    const int t0 = tgrp + NT * n;
+                    if (D <= 16 || lane < 16) {
+                        if (t0 >= a.hdisc && t0 < M - a.hdisc) {
+                            const float f = s0 * a.scale;
+                            outd[(size_t)((t0 - a.hdisc) >> LOGD) * a.out_pitch] = f;
+                            if (SUMS) { sum1 += (double)f; sum2 = fma((double)f, (double)f, sum2); }
+                        }
+                        const int t1 = t0 + L;
+                        if (t1 >= a.hdisc && t1 < M - a.hdisc) {
+                            const float f = s1 * a.scale;
+                            outd[(size_t)((t1 - a.hdisc) >> LOGD) * a.out_pitch] = f;
+                            if (SUMS) { sum1 += (double)f; sum2 = fma((double)f, (double)f, sum2); }
+                        }
+                    }
                 }
-                const int b = a.unit0 / a.nsub + 2 * bp + t;
-                a.segsum[((size_t)(d_begin + (int)j) * a.nblock_total + b) * nchan_total + ochan] = make_double2(a1, a2);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(tbar + 1);  // the tile may be filled again
+                if (SUMS) {
+                    warp_sum_pair(sum1, sum2);
+                    if (lane == 0) ps[g * G::NWARP + q] = make_double2(sum1, sum2);
+                }
+            }
+            if (SUMS) {
+                asm volatile("bar.sync 1, 128;" ::: "memory");
+                if (t < G::NGRP && (t == 0 || has_b)) {
+                    double a1 = 0.0, a2 = 0.0;
+#pragma unroll
+                    for (int w = 0; w < G::NWARP; ++w) {
+                        a1 += ps[t * G::NWARP + w].x;
+                        a2 += ps[t * G::NWARP + w].y;
+                    }
+                    const int b = a.unit0 / a.nsub + 2 * bp + t;
+                    a.segsum[((size_t)(d_begin + (int)j) * a.nblock_total + b) * nchan_total + ochan] = make_double2(a1, a2);
+                }
             }
         };
 #pragma unroll 1
@@ -254,28 +296,20 @@ k_fused_ws(const FusedArgs a, const __grid_constant__ DmParams dmp)
                 tmem_st16(tcol + G::COL_H + 64 * buf + 16 * part, h);
             }
             ws_warp_arrive(full + buf, lane);
-            // the `empty` wait above ordered this warp after pass 0 of trial i - 2 in both FFT groups, which
-            // comes after they handed over the values of trial i - 3
-            if (SUMS && i >= 3u) block_sums(i - 3u);
+            // while the FFT warps work on trial i with the chirp just delivered: the epilogue of trial i - 1
+            if (i >= 1u) epilogue(i - 1u);
         }
-        if (SUMS) {
-            // the last three trials: after every FFT warp has left its loop
-            tmem_fence_before_sync();
-            __syncthreads();
-            const unsigned n = (unsigned)max(0, d_end - d_begin);
-            for (unsigned j = n > 3u ? n - 3u : 0u; j < n; ++j) block_sums(j);
-            return;
-        }
+        if (d_begin < d_end) epilogue((unsigned)(d_end - d_begin) - 1u);
     } else {
         // ------------------------------------------------------------------ FFT groups
         const bool active = role == 0 || has_b;
         const int g = role;
         float4 *ex0 = smem4 + (size_t)g * (G::group_bytes / sizeof(float4)), *ex1 = ex0 + G::EX;
-        float2 *ib = reinterpret_cast<float2 *>(ex0 + 2 * G::EX) + (warp & 3) * G::INTEG;
+        float2 *ib0 = reinterpret_cast<float2 *>(ex0 + 2 * G::EX) + (size_t)(2 * (warp & 3)) * G::INTEG;  // this warp's two tiles
+        uint64_t *tbar = bars + 24 + 4 * (4 * g + q);
         uint64_t *barA0 = bars + 4 * g, *barA1 = barA0 + 1, *barF0 = barA0 + 2, *barF1 = barA0 + 3;
         const int blk = 2 * bp + g;                               // block inside the chunk
         const int ulocal = blk * a.nsub + s;
-        const int b = a.unit0 / a.nsub + blk;                     // block of this execute
         const uint32_t tX = tcol + (uint32_t)(128 * g);
         if (active) {
             // this thread's bins 2j, 2j+1 of both polarisations -> TMEM as (re_e, re_o, im_e, im_o)
@@ -299,56 +333,6 @@ k_fused_ws(const FusedArgs a, const __grid_constant__ DmParams dmp)
         tmem_fence_after_sync();
         asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(G::REGS_FFT));
         if (active) {
-            const int nchan_total = a.nsub * a.nchan;
-            const int ochan = nchan_total - 1 - (s * a.nchan + c);
-            float *out0 = a.out + (size_t)b * a.vdec * a.out_pitch + ochan;
-            const int il = lane & (DG - 1), g0 = lane - il;
-            const int tgrp = (D > 16) ? (t & ~31) : (t - il);  // first sample of a lane's group, before + NT n
-
-            // Second half of the time integration of one trial (the tile was filled at the end of that
-            // trial): one lane sums the D adjacent samples of a row, scales and stores them time-major.
-            // It runs inside the NEXT trial, where its shared-memory and store latencies are covered.
-            auto integrate_store = [&](int dd) {
-                float *outd = out0 + (size_t)dd * (size_t)a.out_stride_dm;
-                float mine[4] = {0.f, 0.f, 0.f, 0.f};  // what this lane stores (two values per kk step)
-#pragma unroll
-                for (int kk = 0; kk < 16 / DG; ++kk) {
-                    const int n = il + DG * kk;
-                    const float4 *row = reinterpret_cast<const float4 *>(ib + n * G::IROW + g0);
-                    P2 acc = pk(0.f, 0.f);
-#pragma unroll
-                    for (int qq = 0; qq < DG / 2; ++qq) {
-                        const float4 f = row[qq];
-                        acc = add2(acc, add2(pk(f.x, f.y), pk(f.z, f.w)));
-                    }
-                    float s0, s1;
-                    upk(acc, s0, s1);
-                    if (D > 16) {
-                        s0 += __shfl_xor_sync(0xffffffffu, s0, 16);
-                        s1 += __shfl_xor_sync(0xffffffffu, s1, 16);
-                    }
-                    const int t0 = tgrp + NT * n;
-                    if (D <= 16 || lane < 16) {
-                        if (t0 >= a.hdisc && t0 < M - a.hdisc) {
-                            const float f = s0 * a.scale;
-                            outd[(size_t)((t0 - a.hdisc) >> LOGD) * a.out_pitch] = f;
-                            mine[(2 * kk) & 3] = f;
-                        }
-                        const int t1 = t0 + L;
-                        if (t1 >= a.hdisc && t1 < M - a.hdisc) {
-                            const float f = s1 * a.scale;
-                            outd[(size_t)((t1 - a.hdisc) >> LOGD) * a.out_pitch] = f;
-                            mine[(2 * kk + 1) & 3] = f;
-                        }
-                    }
-                }
-                // block sums (Alg. 1 l.104): the values go to the chirp warp of this quadrant, which adds them in
-                // fp64; it reads slot dd after the `empty` barrier of trial dd + 1, which this warp reaches later
-                if (SUMS)
-                    fsum[((size_t)((unsigned)(dd - d_begin) & (G::SUM_SLOTS - 1)) * G::NGRP + g) * NT + t] =
-                        make_float4(mine[0], mine[1], mine[2], mine[3]);
-            };
-
 #pragma unroll 1
             for (int d = d_begin; d < d_end; ++d) {
                 const unsigned i = (unsigned)(d - d_begin), buf = i & 1u, par = i & 1u;
@@ -381,7 +365,6 @@ k_fused_ws(const FusedArgs a, const __grid_constant__ DmParams dmp)
                                          ws_pku(hq[cur][4 * rr], hq[cur][4 * rr + 1]), ws_pku(hq[cur][4 * rr + 2], hq[cur][4 * rr + 3]));
                         }
                     }
-                    if (pol == 0 && i != 0u) integrate_store(d - 1);  // the tile of the previous trial
                     PDft<16>::run(v);
                     if (i != 0u) mbar_wait(pol ? barF1 : barF0, par ^ 1u);  // pass-2 loads of trial d-1 are done
                     float4 *dst = (pol ? ex1 : ex0) + j2 * G::RHO + j1 * G::PITCH;
@@ -462,19 +445,22 @@ k_fused_ws(const FusedArgs a, const __grid_constant__ DmParams dmp)
                         }
                     }
                 }
-                // ---- first half of the time integration: the 32 powers of this thread (times t + NT n [+ L])
-                //      go to the warp's tile so that D adjacent samples meet in one lane
-                __syncwarp();  // the reads of the previous trial's tile are done
+                // ---- hand-over to the chirp warp of this quadrant, which integrates and stores: the 32 powers of
+                //      this thread (times t + NT n [+ L]) go to one of the warp's two tiles
+                if (i >= 2u) mbar_wait(tbar + 2 * buf + 1, ((i >> 1) & 1u) ^ 1u);  // tile of trial d - 2 has been read
+                {
+                    float2 *ib = ib0 + (size_t)buf * G::INTEG;
 #pragma unroll
-                for (int k = 0; k < 16; ++k) {
-                    const int n = (k / R2) + U2 * (k % R2);
-                    float2 v2;
-                    upk(pw[k], v2.x, v2.y);
-                    ib[n * G::IROW + lane] = v2;
+                    for (int k = 0; k < 16; ++k) {
+                        const int n = (k / R2) + U2 * (k % R2);
+                        float2 v2;
+                        upk(pw[k], v2.x, v2.y);
+                        ib[n * G::IROW + lane] = v2;
+                    }
                 }
                 __syncwarp();
+                if (lane == 0) mbar_arrive(tbar + 2 * buf);
             }
-            if (d_begin < d_end) integrate_store(d_end - 1);
         }
     }
     tmem_fence_before_sync();
