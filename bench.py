@@ -34,9 +34,10 @@ UNIT = "samples*DM/s"
 # FP32 (non-tensor) peak of a B200: 148 SMs x 128 FP32 lanes x 2 flop/FMA x 1.965 GHz
 # (unit counts and clocks: /opt/skills/guides/B200_PROFILING.md, MEASURED_PEAKS.json sm_max_mhz)
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
-# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per fused-kernel launch from the committed
-# `ncu --set full` capture (profiles/r1_x2_c3.md: 1.085494 + 1.168215 GB; c3, default chunking)
-FUSED_TRAFFIC_BYTES_PER_LAUNCH = {"c3": 2253709000}
+# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of one fused-kernel launch from the committed
+# `ncu --set full` capture (profiles/r2_ws_c3.md: 4.397368 + 4.865498 GB for a launch of 4032 units of c3),
+# per (subband, block) unit; roofline.traffic scales it to the units of a timed launch
+FUSED_TRAFFIC_BYTES_PER_UNIT = {"c3": (4397368000 + 4865498000) / 4032.0}
 
 
 def algorithmic_flops_per_unit_dm(cfg: synth.Config) -> float:
@@ -431,8 +432,9 @@ def main():
     fma_peak = cdmt.cdmt_measure_fp32_peak(scratch, scratch.numel() * 4, 3)
     roofline = {"bound": "alu", "kernel": "k_fused", "achieved": achieved, "peak": FP32_PEAK_TFLOPS,
                 "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
-                "traffic": FUSED_TRAFFIC_BYTES_PER_LAUNCH.get(cfg.name) if not (args.chunk_units or args.dm_tile) else None,
-                "traffic_source": "profiles/r1_x2_c3.md (ncu --set full, one launch)",
+                "traffic": (FUSED_TRAFFIC_BYTES_PER_UNIT[cfg.name] * units_per_step * args.steps / max(1, prof["n_fused"]))
+                           if cfg.name in FUSED_TRAFFIC_BYTES_PER_UNIT and not args.dm_tile else None,
+                "traffic_source": "profiles/r2_ws_c3.md (ncu --set full, one launch of 4032 units, scaled to this launch's units)",
                 "peak_source": "derived: 148 SM x 128 lanes x 2 x 1.965 GHz",
                 "fma_peak_measured_tflops": fma_peak,
                 "ms_per_launch": ms_per_launch, "launches_timed": prof["n_fused"],

@@ -62,16 +62,19 @@ enum { CDMT_REF_CHANNEL = 0, CDMT_REF_SUBBAND = 1 }; /* nu_0 of Eq. 1 (PAPER.md:
 
 /* Tuning knobs for cdmt_plan_set_option (defaults chosen by the library). */
 enum {
-    CDMT_OPT_CHUNK_UNITS = 0, /* (subband, block) units whose spectra are resident at once */
+    CDMT_OPT_CHUNK_UNITS = 0, /* (subband, block) units whose spectra are resident at once (0 = about 4 GiB of
+                                 spectra, a whole and even number of blocks; the workspace holds twice that) */
     CDMT_OPT_DM_TILE = 1,     /* DM trials looped inside one CTA of the fused kernel (0 = all) */
     CDMT_OPT_ACCURATE_SINCOS = 2, /* 1: sincospif instead of the fast approximation */
     CDMT_OPT_PROFILE = 3,     /* 1: record CUDA events round each kernel class (cdmt_profile_read) */
     CDMT_OPT_FUSED_KERNEL = 4, /* fused per-DM kernel: 0 = best applicable (default), 1 = general kernel (any ndec /
                                   overlap), 2 = scalar fast kernel, 3 = packed-FP32 + tensor-memory kernel with the
-                                  even/odd half transforms in the register lanes, 4 = the same with the two
-                                  polarisations in the lanes (16 warps per SM), 5 = kernel 4 software-pipelined
-                                  (chirp of the next trial formed in the shadow of the block barrier); 2 to 5
-                                  make cdmt_execute fail with CDMT_ERR_CUDA where they do not apply */
+                                  even/odd half transforms in the register lanes (k_fused_x2), 4 = the same
+                                  arithmetic warp-specialised: two blocks per CTA share a chirp that dedicated
+                                  warps form and hand over through tensor memory (k_fused_ws; nfft/nchan = 4096),
+                                  5 = packed kernel with the two polarisations in the lanes, chirp of the next
+                                  trial formed in the shadow of the block barrier (k_fused_sp); 2 to 5 make
+                                  cdmt_execute fail with CDMT_ERR_CUDA where they do not apply */
     CDMT_OPT_FORCE_GENERIC = 4, /* older name of the same key (value 1) */
     CDMT_OPT_HOST_GROUP_BLOCKS = 5, /* cdmt_execute_host: blocks staged per group (0 = about 1 GiB of output, an even number) */
     CDMT_OPT_KEEP_TABLES = 6  /* 1: the caller promises that nothing but this plan's executes writes to
@@ -271,7 +274,7 @@ int cdmt_redigitize_sums(cdmt_plan *plan, const float *d_fb, long long fb_stride
  * are exact on integer-valued data and equal to the definition to float32 rounding otherwise.  The plan
  * caches the shift and group tables of the last ddm list it was given (these calls therefore take a
  * non-const plan and, like every other call, must not run concurrently on one plan) and, from the first
- * cdmt_incoherent_dedisperse on, a page-locked copy of them: the call queues two asynchronous copies
+ * cdmt_incoherent_dedisperse on, a page-locked copy of them: the call queues one asynchronous copy
  * from that memory and one kernel on `cuda_stream`, nothing else (capturable into a CUDA graph).
  * Limits (CDMT_ERR_SIZE from all three calls): shift_range <= about 14000 samples (four channels of
  * 256 + shift_range samples must fit shared memory), at most 16 x 65535 trial groups.

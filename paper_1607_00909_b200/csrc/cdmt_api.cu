@@ -223,13 +223,15 @@ static long long nblock_for(const Geometry &g, long long nsamp)
     return nsamp < g.nfft ? 0 : (nsamp - g.nfft) / g.step + 1;
 }
 
-// units resident at once: by default about 1 GiB of spectra
+// units resident at once: by default about 4 GiB of spectra (and as much again for the pass-A buffer).
+// The fused kernel runs one CTA per SM for ~0.4 ms, so a launch of n CTAs loses the unfilled part of
+// its last wave: 4608 CTAs (c3 at 1 GiB) are 31.1 waves on 148 SMs = 2.7 % idle, 32256 are 217.9 = 0.03 %.
 static long long chunk_units_for(const cdmt_plan *p, long long nunits)
 {
     long long c = p->chunk_units;
     if (c <= 0) {
         const long long per_unit = 2LL * p->g.nfft * (long long)sizeof(float2);
-        c = (1LL << 30) / per_unit;
+        c = (4LL << 30) / per_unit;
         if (c < 1) c = 1;
     }
     // grid.x of the fused kernel = chunk * nchan must stay below 2^31

@@ -21,10 +21,16 @@
 // chunks of 32, transposing each chunk's tile [32][256 + range] into shared memory (coalesced float4
 // loads along channels, row length = 1 mod 32 so that the transposing stores are conflict-free); a
 // thread keeps 8 trials x 8 samples (t = lane + 32 i) plus the five run sums in registers and reads 8
-// samples per channel and distinct shift with conflict-free LDS.32.  The table words of a (group,
-// channel) are made warp-uniform for the compiler by a shuffle, so every test on them is a uniform
-// branch.  Measured on c3 (251 fine trials x 96 coherent DMs): 54 ms against 66 ms for the
-// trial-by-trial kernel it replaces (16 x 8 trials: 54 ms, 8 x 8: 58 ms, 4 x 8: 69 ms).
+// samples per channel and distinct shift with conflict-free LDS.32.
+//
+// The first trial's shift s0 of a channel changes every ~90 channels at most (c3: 15 us of delay between
+// neighbouring channels against 1.3 ms samples), so the host cuts every run further into SEGMENTS of
+// channels that also share s0.  A warp walks the segment list of its trial group: inside a segment the
+// window address only moves by one tile row per channel, so the channel loop holds nothing but the
+// loads and adds (no table word, no shuffle, no test per channel), specialised by the run's spread; the
+// segment records (one uint4 per ~30 channels) are read from global memory and made warp-uniform by a
+// shuffle.  Measured on c3 (251 fine trials x 96 coherent DMs): see profiles/; 54 ms for the
+// per-channel table walk this replaces, 66 ms for the trial-by-trial kernel before that.
 #include <algorithm>
 #include <cmath>
 #include <cstdint>
@@ -71,6 +77,8 @@ bool incoherent_plan(const Geometry &g, const double *h_fcen, int nfine, const d
     // groups of up to 8 consecutive trials whose shifts grow by at most 3 samples per trial and 4 in all
     T->groups.clear();
     T->entries.clear();
+    T->segs.clear();
+    T->seg_off.clear();
     int k0 = 0;
     while (k0 < nfine) {
         int n = 1;
@@ -101,8 +109,24 @@ bool incoherent_plan(const Geometry &g, const double *h_fcen, int nfine, const d
         // a run ends where the next channel has another increment pattern, and at the last channel
         for (int j = 0; j < nch; ++j)
             if (j == nch - 1 || T->entries[e0 + j].y != T->entries[e0 + j + 1].y) T->entries[e0 + j].x |= 1u << 28;
+        // segments: maximal channel ranges [c0, c1) with the same first shift and increment pattern;
+        // z = (s0 - smin) | spread << 24 | (the segment closes its run) << 28, w = the pattern
+        T->seg_off.push_back((int)T->segs.size());
+        for (int j = 0; j < nch;) {
+            const uint2 e = T->entries[e0 + j];
+            int j1 = j;
+            while (!(T->entries[e0 + j1].x & (1u << 28)) && (T->entries[e0 + j1 + 1].x & 0xffffffu) == (e.x & 0xffffffu)) ++j1;
+            uint4 sg;
+            sg.x = (unsigned)j;
+            sg.y = (unsigned)(j1 + 1);
+            sg.z = (e.x & 0x07ffffffu) | (T->entries[e0 + j1].x & (1u << 28));
+            sg.w = e.y;
+            T->segs.push_back(sg);
+            j = j1 + 1;
+        }
         k0 += n;
     }
+    T->seg_off.push_back((int)T->segs.size());
     return true;
 }
 
@@ -110,7 +134,7 @@ static size_t ic_align(size_t x) { return (x + 255) & ~(size_t)255; }
 
 size_t incoherent_workspace_bytes(const IncoherentTables &T)
 {
-    return ic_align(T.entries.size() * sizeof(uint2)) + ic_align(T.groups.size() * sizeof(int2));
+    return ic_align(T.segs.size() * sizeof(uint4)) + ic_align(T.seg_off.size() * sizeof(int)) + ic_align(T.groups.size() * sizeof(int2));
 }
 
 // ---------------------------------------------------------------------------------------- device
@@ -119,74 +143,40 @@ struct IcArgs {
     long long fb_stride_dm;
     float *ts;              // [ndm] planes of [nfine] rows of ts_pitch
     long long ts_stride_dm, ts_pitch;
-    const uint2 *entries;   // [ngroups][nch]
+    const uint4 *segs;      // segment records, group after group
+    const int *seg_off;     // [ngroups + 1] first segment of a group
     const int2 *groups;     // [ngroups]
     int nt_in, nt_out, nch, ngroups, cc, tw, vec_in;
     int gpc, tt;            // trial groups and 256-sample time tiles per CTA: gpc * tt <= IC_WARPS warps are live
 };
 
-// Run sums of the distinct shifts O1 and O2 = O1 + 1 of one channel: if spread >= O1 add this lane's
-// 8 samples at s0 + O1 into PA, and if spread >= O2 those at s0 + O2 into PB.  PTX so that the tests
-// stay two-instruction branches (`bra.uni`: every lane holds the same table word) instead of sixteen
-// predicated loads and adds on the common path, where spread is 0 and only the first test executes.
-template <int O1>
-__device__ __forceinline__ void ic_run_add2(float (&PA)[8], float (&PB)[8], unsigned sp, unsigned spread)
+// Run sums over the n channels of a segment: P_o[i] += tile[c][s0 + o + lane + 32 i], o <= SP (the run's spread)
+template <int SP>
+__device__ __forceinline__ void ic_seg_add(float (&P)[IC_MAXSPREAD + 1][8], const float *p, int n, int tw)
 {
-    asm volatile(
-        "{\n\t"
-        ".reg .pred q;\n\t"
-        ".reg .f32 t<8>;\n\t"
-        ".reg .b32 a;\n\t"
-        "setp.lt.u32 q, %17, %18;\n\t"
-        "@q bra.uni IC_END;\n\t"
-        "add.u32 a, %16, %20;\n\t"
-        "ld.shared.f32 t0, [a];\n\t"
-        "ld.shared.f32 t1, [a+128];\n\t"
-        "ld.shared.f32 t2, [a+256];\n\t"
-        "ld.shared.f32 t3, [a+384];\n\t"
-        "ld.shared.f32 t4, [a+512];\n\t"
-        "ld.shared.f32 t5, [a+640];\n\t"
-        "ld.shared.f32 t6, [a+768];\n\t"
-        "ld.shared.f32 t7, [a+896];\n\t"
-        "add.f32 %0, %0, t0;\n\t"
-        "add.f32 %1, %1, t1;\n\t"
-        "add.f32 %2, %2, t2;\n\t"
-        "add.f32 %3, %3, t3;\n\t"
-        "add.f32 %4, %4, t4;\n\t"
-        "add.f32 %5, %5, t5;\n\t"
-        "add.f32 %6, %6, t6;\n\t"
-        "add.f32 %7, %7, t7;\n\t"
-        "setp.lt.u32 q, %17, %19;\n\t"
-        "@q bra.uni IC_END;\n\t"
-        "add.u32 a, %16, %21;\n\t"
-        "ld.shared.f32 t0, [a];\n\t"
-        "ld.shared.f32 t1, [a+128];\n\t"
-        "ld.shared.f32 t2, [a+256];\n\t"
-        "ld.shared.f32 t3, [a+384];\n\t"
-        "ld.shared.f32 t4, [a+512];\n\t"
-        "ld.shared.f32 t5, [a+640];\n\t"
-        "ld.shared.f32 t6, [a+768];\n\t"
-        "ld.shared.f32 t7, [a+896];\n\t"
-        "add.f32 %8, %8, t0;\n\t"
-        "add.f32 %9, %9, t1;\n\t"
-        "add.f32 %10, %10, t2;\n\t"
-        "add.f32 %11, %11, t3;\n\t"
-        "add.f32 %12, %12, t4;\n\t"
-        "add.f32 %13, %13, t5;\n\t"
-        "add.f32 %14, %14, t6;\n\t"
-        "add.f32 %15, %15, t7;\n\t"
-        "IC_END:\n\t"
-        "}"
-        : "+f"(PA[0]), "+f"(PA[1]), "+f"(PA[2]), "+f"(PA[3]), "+f"(PA[4]), "+f"(PA[5]), "+f"(PA[6]), "+f"(PA[7]),
-          "+f"(PB[0]), "+f"(PB[1]), "+f"(PB[2]), "+f"(PB[3]), "+f"(PB[4]), "+f"(PB[5]), "+f"(PB[6]), "+f"(PB[7])
-        : "r"(sp), "r"(spread), "n"(O1), "n"(O1 + 1), "n"(4 * O1), "n"(4 * (O1 + 1))
-        : "memory");
+#pragma unroll 1
+    for (int c = 0; c < n; ++c) {
+#pragma unroll
+        for (int o = 0; o <= SP; ++o)
+#pragma unroll
+            for (int i = 0; i < 8; ++i) P[o][i] += p[32 * i + o];
+        p += tw;
+    }
+}
+
+__device__ __forceinline__ uint4 ic_uniform(uint4 v)
+{
+    // the record is the same in every lane; the shuffles let the compiler know it (uniform branches)
+    v.x = __shfl_sync(0xffffffffu, v.x, 0);
+    v.y = __shfl_sync(0xffffffffu, v.y, 0);
+    v.z = __shfl_sync(0xffffffffu, v.z, 0);
+    v.w = __shfl_sync(0xffffffffu, v.w, 0);
+    return v;
 }
 
 // grid (ceil(nt_out / (256 tt)), ceil(ngroups / gpc), ndm), 32 IC_WARPS threads; warp w works on trial group
 // w % gpc and time tile w / gpc of the CTA (few trial groups: several time tiles share one staged tile,
 // so that the warps stay busy and the halo is re-read less).  Dynamic shared memory: float tile[cc][tw]
-// and uint2 tab[gpc][cc]
 template <bool MULTI>   // false: gpc = IC_WARPS, tt = 1 as compile-time constants (the common, register-tight case)
 __global__ void __launch_bounds__(32 * IC_WARPS, 1) k_incoherent(const IcArgs a)
 {
@@ -194,7 +184,6 @@ __global__ void __launch_bounds__(32 * IC_WARPS, 1) k_incoherent(const IcArgs a)
     extern __shared__ float4 ic_smem4[];
     float *tile = reinterpret_cast<float *>(ic_smem4);
     const int cc = a.cc, tw = a.tw, quads = cc >> 2;
-    uint2 *tab = reinterpret_cast<uint2 *>(tile + (((size_t)cc * tw + 3) & ~(size_t)3));
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tbase = blockIdx.x * IC_TILE * tt;           // first sample of the staged tile
     const int gsel = MULTI ? warp % gpc : warp, sub = MULTI ? warp / gpc : 0;
@@ -216,6 +205,13 @@ __global__ void __launch_bounds__(32 * IC_WARPS, 1) k_incoherent(const IcArgs a)
     for (int o = 0; o <= IC_MAXSPREAD; ++o)
 #pragma unroll
         for (int i = 0; i < 8; ++i) P[o][i] = 0.f;
+
+    int cur = 0, cur_end = 0;
+    if (live) {
+        cur = a.seg_off[grp];
+        cur_end = a.seg_off[grp + 1];
+    }
+    uint4 sg = cur < cur_end ? ic_uniform(__ldg(a.segs + cur)) : make_uint4(0x7fffffffu, 0x7fffffffu, 0u, 0u);
 
     for (int c0 = 0; c0 < a.nch; c0 += cc) {
         __syncthreads();  // the previous chunk has been consumed
@@ -250,36 +246,27 @@ __global__ void __launch_bounds__(32 * IC_WARPS, 1) k_incoherent(const IcArgs a)
                 }
             }
         }
-        for (int e = tid; e < gpc * cc; e += 32 * IC_WARPS) {
-            const int w = e / cc, c = e % cc;
-            const int gw = blockIdx.y * gpc + w;
-            uint2 v = make_uint2(0u, 0u);
-            if (gw < a.ngroups && c0 + c < a.nch) v = a.entries[(size_t)gw * a.nch + c0 + c];
-            tab[w * cc + c] = v;
-        }
         __syncthreads();
         if (!live) continue;
-        // ---- add the chunk's channels into the run sums; at the end of a run, into the trials
-#pragma unroll 1
-        for (int c = 0; c < cc; ++c) {
-            const uint2 e0 = tab[gsel * cc + c];
-            // the table words are the same in every lane; the shuffles let the compiler know it
-            uint2 e;
-            e.x = __shfl_sync(0xffffffffu, e0.x, 0);
-            e.y = __shfl_sync(0xffffffffu, e0.y, 0);
-            const unsigned s0 = e.x & 0xffffffu, spread = (e.x >> 24) & 7u;
-            const float *p = tile + (size_t)c * tw + s0 + lane + sub * IC_TILE;
-#pragma unroll
-            for (int i = 0; i < 8; ++i) P[0][i] += p[32 * i];
-            const unsigned sp = (unsigned)__cvta_generic_to_shared(p);
-            ic_run_add2<1>(P[1], P[2], sp, spread);
-            ic_run_add2<3>(P[3], P[4], sp, spread);
-            if (e.x & (1u << 28)) {
+        // ---- the segments of this warp's trial group that reach into the chunk
+        while ((int)sg.x < c0 + cc) {
+            const int a0 = max((int)sg.x, c0), a1 = min((int)sg.y, c0 + cc);
+            const unsigned s0 = sg.z & 0xffffffu, spread = (sg.z >> 24) & 7u;
+            const float *p = tile + (size_t)(a0 - c0) * tw + s0 + lane + sub * IC_TILE;
+            switch (spread) {
+            case 0: ic_seg_add<0>(P, p, a1 - a0, tw); break;
+            case 1: ic_seg_add<1>(P, p, a1 - a0, tw); break;
+            case 2: ic_seg_add<2>(P, p, a1 - a0, tw); break;
+            case 3: ic_seg_add<3>(P, p, a1 - a0, tw); break;
+            default: ic_seg_add<4>(P, p, a1 - a0, tw); break;
+            }
+            if ((int)sg.y > c0 + cc) break;   // goes on in the next chunk
+            if (sg.z & (1u << 28)) {
                 // end of the run: trial k takes the sum at its cumulative increment o_k
                 unsigned o = 0;
 #pragma unroll
                 for (int k = 0; k < IC_GROUP; ++k) {
-                    if (k > 0) o += (e.y >> (2 * k)) & 3u;
+                    if (k > 0) o += (sg.w >> (2 * k)) & 3u;
                     if (o == 0u) {
 #pragma unroll
                         for (int i = 0; i < 8; ++i) acc[k][i] += P[0][i];
@@ -302,6 +289,192 @@ __global__ void __launch_bounds__(32 * IC_WARPS, 1) k_incoherent(const IcArgs a)
 #pragma unroll
                     for (int i = 0; i < 8; ++i) P[oo][i] = 0.f;
             }
+            ++cur;
+            sg = cur < cur_end ? ic_uniform(__ldg(a.segs + cur)) : make_uint4(0x7fffffffu, 0x7fffffffu, 0u, 0u);
+        }
+    }
+    if (!live) return;
+    const int2 gi = a.groups[grp];
+    float *out = a.ts + (size_t)blockIdx.z * (size_t)a.ts_stride_dm;
+#pragma unroll
+    for (int k = 0; k < IC_GROUP; ++k) {
+        if (k >= gi.y) break;
+        float *row = out + (size_t)(gi.x + k) * (size_t)a.ts_pitch;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const int t = t0 + lane + 32 * i;
+            if (t < a.nt_out) row[t] = acc[k][i];
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// k_incoherent_v4: the same sums for filterbanks whose rows can be read in 16-byte pieces (channel count
+// a multiple of 4, aligned planes) and whose shift range lets two tiles fit shared memory.
+//
+//  * The tile keeps the filterbank's own order, [time][32 channels] = 128-byte rows, and is filled by
+//    16-byte cp.async copies (no registers, no transposing stores) into one of TWO buffers: the copies of
+//    chunk c+1 fly while chunk c is summed.  (One CTA of 16 warps x 128 registers fills an SM, so in
+//    k_incoherent the global loads of a chunk -- two batches, ~1.5 us each -- are exposed once per chunk,
+//    about as long as the summing itself.)
+//  * The 16-byte pieces of a row are XOR-swizzled with the row number (piece j of row r sits at
+//    j ^ (r & 7)), so that a quarter warp -- 8 lanes = 8 consecutive time samples of one channel quad --
+//    reads 8 different pieces: LDS.128 without bank conflicts.  A lane therefore takes FOUR channels of a
+//    sample at once (they share the segment's first shift) and adds (x + y) + (z + w) into the run sum:
+//    a quarter of the shared-memory instructions for the same bytes.  Channels in front of / behind the
+//    4-aligned part of a segment are taken one by one (LDS.32, 4-way conflicts, rare).
+//  * Everything else -- trial groups, runs, segments, end-of-run hand-over -- as in k_incoherent; the
+//    additions of a run happen in another order (pairs inside a quad first), exact on integer data.
+// ------------------------------------------------------------------------------------------------
+constexpr int IC4_CC = 32;   // channels per chunk = one 128-byte row
+
+__device__ __forceinline__ void ic_cp16(unsigned dst, const void *src, int bytes)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(bytes) : "memory");
+}
+
+// P_o[i] += sum of the four channels of quad j at rows s0 + o + lane + 32 i (+ the warp's time tile)
+template <int SP>
+__device__ __forceinline__ void ic4_quads(float (&P)[IC_MAXSPREAD + 1][8], unsigned rowaddr, unsigned row7, int j0, int nq)
+{
+#pragma unroll 1
+    for (int j = j0; j < j0 + nq; ++j) {
+#pragma unroll
+        for (int o = 0; o <= SP; ++o) {
+            // row r = r_lane + o: its swizzle term is ((row7 + o) & 7); 32 i more rows do not change it
+            const unsigned a = rowaddr + 128u * o + ((((unsigned)j ^ (row7 + o)) & 7u) << 4);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                float x, y, z, w;
+                asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(x), "=f"(y), "=f"(z), "=f"(w) : "r"(a + 4096u * i));
+                P[o][i] += (x + y) + (z + w);
+            }
+        }
+    }
+}
+template <int SP>
+__device__ __forceinline__ void ic4_single(float (&P)[IC_MAXSPREAD + 1][8], unsigned rowaddr, unsigned row7, int c)
+{
+#pragma unroll
+    for (int o = 0; o <= SP; ++o) {
+        const unsigned a = rowaddr + 128u * o + ((((unsigned)(c >> 2) ^ (row7 + o)) & 7u) << 4) + 4u * (c & 3);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            float x;
+            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(x) : "r"(a + 4096u * i));
+            P[o][i] += x;
+        }
+    }
+}
+// channels [a0, a1) of the staged chunk (chunk-relative), all with the first shift of `rowaddr`
+template <int SP>
+__device__ __forceinline__ void ic4_seg_add(float (&P)[IC_MAXSPREAD + 1][8], unsigned rowaddr, unsigned row7, int a0, int a1)
+{
+    while ((a0 & 3) && a0 < a1) ic4_single<SP>(P, rowaddr, row7, a0++);
+    const int nq = (a1 - a0) >> 2;
+    if (nq > 0) ic4_quads<SP>(P, rowaddr, row7, a0 >> 2, nq);
+    for (int c = a0 + 4 * nq; c < a1; ++c) ic4_single<SP>(P, rowaddr, row7, c);
+}
+
+template <bool MULTI>
+__global__ void __launch_bounds__(32 * IC_WARPS, 1) k_incoherent_v4(const IcArgs a)
+{
+    const int gpc = MULTI ? a.gpc : IC_WARPS, tt = MULTI ? a.tt : 1;
+    extern __shared__ float4 ic_smem4[];
+    const int rows = a.tw;                                  // input samples staged per chunk: range + 256 tt
+    const unsigned tile0 = (unsigned)__cvta_generic_to_shared(ic_smem4), tile_bytes = 128u * (unsigned)rows;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tbase = blockIdx.x * IC_TILE * tt;
+    const int gsel = MULTI ? warp % gpc : warp, sub = MULTI ? warp / gpc : 0;
+    const int t0 = tbase + sub * IC_TILE;
+    const int grp = blockIdx.y * gpc + gsel;
+    const bool live = sub < tt && grp < a.ngroups && t0 < a.nt_out;
+    const float *fb = a.fb + (size_t)blockIdx.z * (size_t)a.fb_stride_dm;
+
+    float acc[IC_GROUP][8];
+    float P[IC_MAXSPREAD + 1][8];
+#pragma unroll
+    for (int k = 0; k < IC_GROUP; ++k)
+#pragma unroll
+        for (int i = 0; i < 8; ++i) acc[k][i] = 0.f;
+#pragma unroll
+    for (int o = 0; o <= IC_MAXSPREAD; ++o)
+#pragma unroll
+        for (int i = 0; i < 8; ++i) P[o][i] = 0.f;
+
+    int cur = 0, cur_end = 0;
+    if (live) {
+        cur = a.seg_off[grp];
+        cur_end = a.seg_off[grp + 1];
+    }
+    uint4 sg = cur < cur_end ? ic_uniform(__ldg(a.segs + cur)) : make_uint4(0x7fffffffu, 0x7fffffffu, 0u, 0u);
+
+    // 16-byte pieces of chunk c0 -> buffer `buf`; rows beyond the filterbank and channels beyond nch are zero
+    auto stage = [&](int c0, int buf) {
+        const unsigned dst0 = tile0 + (unsigned)buf * tile_bytes;
+        for (int e = tid; e < rows * 8; e += 32 * IC_WARPS) {
+            const int r = e >> 3, j = e & 7, t = tbase + r, c = c0 + 4 * j;
+            const bool ok = t < a.nt_in && c < a.nch;      // nch is a multiple of 4: a quad is in or out
+            const float *src = ok ? fb + (size_t)t * a.nch + c : fb;
+            ic_cp16(dst0 + 128u * r + ((unsigned)(j ^ (r & 7)) << 4), src, ok ? 16 : 0);
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+
+    stage(0, 0);
+    int buf = 0;
+    for (int c0 = 0; c0 < a.nch; c0 += IC4_CC, buf ^= 1) {
+        __syncthreads();                                   // the other buffer has been consumed
+        if (c0 + IC4_CC < a.nch) {
+            stage(c0 + IC4_CC, buf ^ 1);
+            asm volatile("cp.async.wait_group 1;" ::: "memory");
+        } else {
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+        }
+        __syncthreads();                                   // every thread's pieces of this chunk have landed
+        if (!live) continue;
+        while ((int)sg.x < c0 + IC4_CC) {
+            const int a0 = max((int)sg.x, c0) - c0, a1 = min((int)sg.y, c0 + IC4_CC) - c0;
+            const unsigned s0 = sg.z & 0xffffffu, spread = (sg.z >> 24) & 7u;
+            const unsigned r_lane = s0 + lane + sub * IC_TILE;
+            const unsigned rowaddr = tile0 + (unsigned)buf * tile_bytes + 128u * r_lane, row7 = r_lane & 7u;
+            switch (spread) {
+            case 0: ic4_seg_add<0>(P, rowaddr, row7, a0, a1); break;
+            case 1: ic4_seg_add<1>(P, rowaddr, row7, a0, a1); break;
+            case 2: ic4_seg_add<2>(P, rowaddr, row7, a0, a1); break;
+            case 3: ic4_seg_add<3>(P, rowaddr, row7, a0, a1); break;
+            default: ic4_seg_add<4>(P, rowaddr, row7, a0, a1); break;
+            }
+            if ((int)sg.y > c0 + IC4_CC) break;
+            if (sg.z & (1u << 28)) {
+                unsigned o = 0;
+#pragma unroll
+                for (int k = 0; k < IC_GROUP; ++k) {
+                    if (k > 0) o += (sg.w >> (2 * k)) & 3u;
+                    if (o == 0u) {
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) acc[k][i] += P[0][i];
+                    } else if (o == 1u) {
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) acc[k][i] += P[1][i];
+                    } else if (o == 2u) {
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) acc[k][i] += P[2][i];
+                    } else if (o == 3u) {
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) acc[k][i] += P[3][i];
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) acc[k][i] += P[4][i];
+                    }
+                }
+#pragma unroll
+                for (int oo = 0; oo <= IC_MAXSPREAD; ++oo)
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) P[oo][i] = 0.f;
+            }
+            ++cur;
+            sg = cur < cur_end ? ic_uniform(__ldg(a.segs + cur)) : make_uint4(0x7fffffffu, 0x7fffffffu, 0u, 0u);
         }
     }
     if (!live) return;
@@ -353,7 +526,7 @@ bool incoherent_config(const IncoherentTables &T, int *cc_out, int *tw_out, int 
     int tt = IC_WARPS / gpc;
     for (;; --tt) {
         const int tw = ((T.range + tt * IC_TILE + 30) & ~31) + 1;   // >= range + 256 tt and = 1 mod 32
-        auto smem_for = [&](int cc) { return sizeof(float) * (((size_t)cc * tw + 3) & ~(size_t)3) + sizeof(uint2) * gpc * cc; };
+        auto smem_for = [&](int cc) { return sizeof(float) * (((size_t)cc * tw + 3) & ~(size_t)3); };
         // channels per chunk: 32 if the tile stays below 72 KB, else fewer time tiles; at one time tile
         // whatever number of channels fits shared memory
         int cc = 0;
@@ -373,6 +546,25 @@ bool incoherent_config(const IncoherentTables &T, int *cc_out, int *tw_out, int 
     }
 }
 
+// k_incoherent_v4: trial groups and time tiles per CTA as above; two tiles of (range + 256 tt) rows of 128 bytes
+static bool incoherent_config_v4(const IncoherentTables &T, int *rows_out, int *gpc_out, int *tt_out, size_t *smem_out)
+{
+    const int ngroups = (int)T.groups.size();
+    if (ngroups < 1) return false;
+    const int ny = (ngroups + IC_WARPS - 1) / IC_WARPS;
+    if (ny > 65535) return false;
+    const int gpc = (ngroups + ny - 1) / ny;
+    for (int tt = IC_WARPS / gpc; tt >= 1; --tt) {
+        const int rows = T.range + tt * IC_TILE;
+        const size_t smem = 2 * (size_t)rows * 128;
+        if (smem <= (tt > 1 ? 160u : 200u) * 1024) {
+            *rows_out = rows; *gpc_out = gpc; *tt_out = tt; *smem_out = smem;
+            return true;
+        }
+    }
+    return false;
+}
+
 void incoherent_release(IncoherentTables *T)
 {
     if (T->pinned) cudaFreeHost(T->pinned);
@@ -386,29 +578,44 @@ cudaError_t launch_incoherent(const Geometry &g, IncoherentTables &T, const floa
     const int nch = T.nch, ngroups = (int)T.groups.size();
     const long long nt_out = nt_in - T.range;
     char *ws = reinterpret_cast<char *>(d_workspace);
-    const size_t nb_e = T.entries.size() * sizeof(uint2), nb_g = T.groups.size() * sizeof(int2);
-    uint2 *d_entries = reinterpret_cast<uint2 *>(ws);
-    int2 *d_groups = reinterpret_cast<int2 *>(ws + ic_align(nb_e));
-    // the tables travel from page-locked memory the plan keeps for them: a plain asynchronous copy on the
+    const size_t nb_s = T.segs.size() * sizeof(uint4), nb_o = T.seg_off.size() * sizeof(int), nb_g = T.groups.size() * sizeof(int2);
+    const size_t off_o = ic_align(nb_s), off_g = off_o + ic_align(nb_o), total = off_g + nb_g;
+    // the tables travel from page-locked memory the plan keeps for them: one plain asynchronous copy on the
     // caller's stream, also inside a stream capture
     if (!T.pinned) {
-        cudaError_t e = cudaMallocHost(&T.pinned, ic_align(nb_e) + nb_g);
+        cudaError_t e = cudaMallocHost(&T.pinned, total);
         if (e != cudaSuccess) return e;
-        memcpy(T.pinned, T.entries.data(), nb_e);
-        memcpy(static_cast<char *>(T.pinned) + ic_align(nb_e), T.groups.data(), nb_g);
+        memset(T.pinned, 0, total);
+        memcpy(T.pinned, T.segs.data(), nb_s);
+        memcpy(static_cast<char *>(T.pinned) + off_o, T.seg_off.data(), nb_o);
+        memcpy(static_cast<char *>(T.pinned) + off_g, T.groups.data(), nb_g);
     }
-    cudaError_t e = cudaMemcpyAsync(d_entries, T.pinned, nb_e, cudaMemcpyHostToDevice, st);
-    if (e != cudaSuccess) return e;
-    e = cudaMemcpyAsync(d_groups, static_cast<char *>(T.pinned) + ic_align(nb_e), nb_g, cudaMemcpyHostToDevice, st);
+    cudaError_t e = cudaMemcpyAsync(ws, T.pinned, total, cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return e;
 
     IcArgs a;
     a.fb = d_fb; a.fb_stride_dm = fb_stride_dm; a.ts = d_ts; a.ts_stride_dm = ts_stride_dm; a.ts_pitch = ts_pitch;
-    a.entries = d_entries; a.groups = d_groups;
+    a.segs = reinterpret_cast<const uint4 *>(ws);
+    a.seg_off = reinterpret_cast<const int *>(ws + off_o);
+    a.groups = reinterpret_cast<const int2 *>(ws + off_g);
     a.nt_in = (int)nt_in; a.nt_out = (int)nt_out; a.nch = nch; a.ngroups = ngroups;
     size_t smem = 0;
-    if (!incoherent_config(T, &a.cc, &a.tw, &a.gpc, &a.tt, &smem)) return cudaErrorInvalidValue;
     a.vec_in = (nch % 4 == 0 && fb_stride_dm % 4 == 0 && (reinterpret_cast<uintptr_t>(d_fb) & 15) == 0) ? 1 : 0;
+    // rows readable in 16-byte pieces and two tiles in shared memory: the cp.async / LDS.128 kernel
+    if (a.vec_in && incoherent_config_v4(T, &a.tw, &a.gpc, &a.tt, &smem)) {
+        a.cc = IC4_CC;
+        const bool multi = !(a.gpc == IC_WARPS && a.tt == 1);
+        e = multi ? cudaFuncSetAttribute(k_incoherent_v4<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
+                  : cudaFuncSetAttribute(k_incoherent_v4<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        dim3 grid((unsigned)((nt_out + IC_TILE * a.tt - 1) / (IC_TILE * a.tt)), (unsigned)((ngroups + a.gpc - 1) / a.gpc), (unsigned)g.ndm);
+        if (multi) k_incoherent_v4<true><<<grid, 32 * IC_WARPS, smem, st>>>(a);
+        else k_incoherent_v4<false><<<grid, 32 * IC_WARPS, smem, st>>>(a);
+        e = cudaGetLastError();
+        if (e == cudaSuccess) ++*launches;
+        return e;
+    }
+    if (!incoherent_config(T, &a.cc, &a.tw, &a.gpc, &a.tt, &smem)) return cudaErrorInvalidValue;
     const bool multi = !(a.gpc == IC_WARPS && a.tt == 1);
     e = multi ? cudaFuncSetAttribute(k_incoherent<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
               : cudaFuncSetAttribute(k_incoherent<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

@@ -76,8 +76,11 @@ struct IncoherentTables {            // host side, owned by the plan (must outli
     int smin = 0, range = 0;         // extremes of the shift table: range = smax - smin
     std::vector<int> shifts;         // [nfine][nch] samples, channel order of the filterbank (descending)
     std::vector<uint2> entries;      // [ngroups][nch]: x = first trial's shift - smin, y = 2-bit increments
+    std::vector<uint4> segs;         // per group: channel ranges [x, y) that share the first shift and the pattern;
+                                     // z = first shift - smin | spread << 24 | closes-its-run << 28, w = 2-bit increments
+    std::vector<int> seg_off;        // [ngroups + 1]: first segment of a group
     std::vector<int2> groups;        // [ngroups]: (first trial, number of trials <= 8)
-    void *pinned = nullptr;          // page-locked copy of entries + groups (made by the first dedisperse)
+    void *pinned = nullptr;          // page-locked copy of segs + seg_off + groups (made by the first dedisperse)
 };
 // Fills the tables; returns false if ddm is not ascending.
 bool incoherent_plan(const Geometry &g, const double *h_fcen, int nfine, const double *ddm, IncoherentTables *T);
