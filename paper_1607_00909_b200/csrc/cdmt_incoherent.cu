@@ -29,11 +29,14 @@
 // window address only moves by one tile row per channel, so the channel loop holds nothing but the
 // loads and adds (no table word, no shuffle, no test per channel), specialised by the run's spread; the
 // segment records (one uint4 per ~30 channels) are read from global memory and made warp-uniform by a
-// shuffle.  Measured on c3 (251 fine trials x 96 coherent DMs): see profiles/; 54 ms for the
-// per-channel table walk this replaces, 66 ms for the trial-by-trial kernel before that.
+// shuffle.  k_incoherent below is the general form (any channel count and alignment, shift ranges up to
+// ~14 000 samples); k_incoherent_v4 further down is the fast form for filterbanks whose rows can be read
+// in 16-byte pieces.  Measured on c3 (251 fine trials x 96 coherent DMs): 41.5 ms (k_incoherent_v4) against
+// 54 ms for the per-channel table walk of round 1 and 66 ms for the trial-by-trial kernel before that.
 #include <algorithm>
 #include <cmath>
 #include <cstdint>
+#include <cstdlib>
 #include <cstring>
 
 #include "cdmt_internal.h"
@@ -109,6 +112,28 @@ bool incoherent_plan(const Geometry &g, const double *h_fcen, int nfine, const d
         // a run ends where the next channel has another increment pattern, and at the last channel
         for (int j = 0; j < nch; ++j)
             if (j == nch - 1 || T->entries[e0 + j].y != T->entries[e0 + j + 1].y) T->entries[e0 + j].x |= 1u << 28;
+        k0 += n;
+    }
+    // Heaviest groups first: the 16 groups of a CTA meet at a block barrier once per chunk, so a CTA runs
+    // at the pace of its slowest warp.  The work of a group -- (1 + spread) window reads per channel plus
+    // the hand-over at every run end -- grows with |ddm| (offsets near zero move no channel by a sample),
+    // so groups sorted by work share a CTA with their like.  (Each group carries its own first trial, so
+    // the order of the records is free.)
+    const int ngroups = (int)T->groups.size();
+    std::vector<double> work((size_t)ngroups, 0.0);
+    for (int gi = 0; gi < ngroups; ++gi)
+        for (int j = 0; j < nch; ++j) {
+            const uint2 e = T->entries[(size_t)gi * nch + j];
+            work[gi] += 1.0 + (double)((e.x >> 24) & 7u) + ((e.x & (1u << 28)) ? 8.0 : 0.0);
+        }
+    std::vector<int> order((size_t)ngroups);
+    for (int gi = 0; gi < ngroups; ++gi) order[gi] = gi;
+    std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return work[x] > work[y]; });
+    std::vector<int2> sorted_groups;
+    sorted_groups.reserve(ngroups);
+    for (int gi : order) {
+        sorted_groups.push_back(T->groups[gi]);
+        const size_t e0 = (size_t)gi * nch;
         // segments: maximal channel ranges [c0, c1) with the same first shift and increment pattern;
         // z = (s0 - smin) | spread << 24 | (the segment closes its run) << 28, w = the pattern
         T->seg_off.push_back((int)T->segs.size());
@@ -124,8 +149,8 @@ bool incoherent_plan(const Geometry &g, const double *h_fcen, int nfine, const d
             T->segs.push_back(sg);
             j = j1 + 1;
         }
-        k0 += n;
     }
+    T->groups.swap(sorted_groups);
     T->seg_off.push_back((int)T->segs.size());
     return true;
 }
@@ -321,8 +346,9 @@ __global__ void __launch_bounds__(32 * IC_WARPS, 1) k_incoherent(const IcArgs a)
 //    j ^ (r & 7)), so that a quarter warp -- 8 lanes = 8 consecutive time samples of one channel quad --
 //    reads 8 different pieces: LDS.128 without bank conflicts.  A lane therefore takes FOUR channels of a
 //    sample at once (they share the segment's first shift) and adds (x + y) + (z + w) into the run sum:
-//    a quarter of the shared-memory instructions for the same bytes.  Channels in front of / behind the
-//    4-aligned part of a segment are taken one by one (LDS.32, 4-way conflicts, rare).
+//    a quarter of the shared-memory instructions for the same bytes.  Where a segment starts or ends inside
+//    a quad, the same 16-byte load is used and the channels of the neighbouring segment are replaced by
+//    zeros (single LDS.32 column reads would meet 4-way bank conflicts in this layout).
 //  * Everything else -- trial groups, runs, segments, end-of-run hand-over -- as in k_incoherent; the
 //    additions of a run happen in another order (pairs inside a quad first), exact on integer data.
 // ------------------------------------------------------------------------------------------------
@@ -334,8 +360,8 @@ __device__ __forceinline__ void ic_cp16(unsigned dst, const void *src, int bytes
 }
 
 // P_o[i] += sum of the four channels of quad j at rows s0 + o + lane + 32 i (+ the warp's time tile)
-template <int SP>
-__device__ __forceinline__ void ic4_quads(float (&P)[IC_MAXSPREAD + 1][8], unsigned rowaddr, unsigned row7, int j0, int nq)
+template <int SP, int NS>
+__device__ __forceinline__ void ic4_quads(float (&P)[IC_MAXSPREAD + 1][NS], unsigned rowaddr, unsigned row7, int j0, int nq)
 {
 #pragma unroll 1
     for (int j = j0; j < j0 + nq; ++j) {
@@ -344,7 +370,7 @@ __device__ __forceinline__ void ic4_quads(float (&P)[IC_MAXSPREAD + 1][8], unsig
             // row r = r_lane + o: its swizzle term is ((row7 + o) & 7); 32 i more rows do not change it
             const unsigned a = rowaddr + 128u * o + ((((unsigned)j ^ (row7 + o)) & 7u) << 4);
 #pragma unroll
-            for (int i = 0; i < 8; ++i) {
+            for (int i = 0; i < NS; ++i) {
                 float x, y, z, w;
                 asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(x), "=f"(y), "=f"(z), "=f"(w) : "r"(a + 4096u * i));
                 P[o][i] += (x + y) + (z + w);
@@ -352,62 +378,76 @@ __device__ __forceinline__ void ic4_quads(float (&P)[IC_MAXSPREAD + 1][8], unsig
         }
     }
 }
-template <int SP>
-__device__ __forceinline__ void ic4_single(float (&P)[IC_MAXSPREAD + 1][8], unsigned rowaddr, unsigned row7, int c)
+// a quad of which only channels [lo, hi) belong to the segment: the same LDS.128, the other components
+// are replaced by zero (lo, hi are warp-uniform, so the selects cost no divergence)
+template <int SP, int NS>
+__device__ __forceinline__ void ic4_partial(float (&P)[IC_MAXSPREAD + 1][NS], unsigned rowaddr, unsigned row7, int j, int lo, int hi)
 {
+    const bool m0 = lo <= 0 && 0 < hi, m1 = lo <= 1 && 1 < hi, m2 = lo <= 2 && 2 < hi, m3 = lo <= 3 && 3 < hi;
 #pragma unroll
     for (int o = 0; o <= SP; ++o) {
-        const unsigned a = rowaddr + 128u * o + ((((unsigned)(c >> 2) ^ (row7 + o)) & 7u) << 4) + 4u * (c & 3);
+        const unsigned a = rowaddr + 128u * o + ((((unsigned)j ^ (row7 + o)) & 7u) << 4);
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
-            float x;
-            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(x) : "r"(a + 4096u * i));
-            P[o][i] += x;
+        for (int i = 0; i < NS; ++i) {
+            float x, y, z, w;
+            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(x), "=f"(y), "=f"(z), "=f"(w) : "r"(a + 4096u * i));
+            P[o][i] += ((m0 ? x : 0.f) + (m1 ? y : 0.f)) + ((m2 ? z : 0.f) + (m3 ? w : 0.f));
         }
     }
 }
 // channels [a0, a1) of the staged chunk (chunk-relative), all with the first shift of `rowaddr`
-template <int SP>
-__device__ __forceinline__ void ic4_seg_add(float (&P)[IC_MAXSPREAD + 1][8], unsigned rowaddr, unsigned row7, int a0, int a1)
+template <int SP, int NS>
+__device__ __forceinline__ void ic4_seg_add(float (&P)[IC_MAXSPREAD + 1][NS], unsigned rowaddr, unsigned row7, int a0, int a1)
 {
-    while ((a0 & 3) && a0 < a1) ic4_single<SP>(P, rowaddr, row7, a0++);
+    if (a0 & 3) {   // head: the rest of the quad a0 sits in (or the whole segment, if it ends inside that quad)
+        const int qe = min((a0 | 3) + 1, a1);
+        ic4_partial<SP, NS>(P, rowaddr, row7, a0 >> 2, a0 & 3, qe - (a0 & ~3));
+        a0 = qe;
+    }
     const int nq = (a1 - a0) >> 2;
-    if (nq > 0) ic4_quads<SP>(P, rowaddr, row7, a0 >> 2, nq);
-    for (int c = a0 + 4 * nq; c < a1; ++c) ic4_single<SP>(P, rowaddr, row7, c);
+    if (nq > 0) ic4_quads<SP, NS>(P, rowaddr, row7, a0 >> 2, nq);
+    a0 += 4 * nq;
+    if (a0 < a1) ic4_partial<SP, NS>(P, rowaddr, row7, a0 >> 2, 0, a1 - a0);
 }
 
-template <bool MULTI>
-__global__ void __launch_bounds__(32 * IC_WARPS, 1) k_incoherent_v4(const IcArgs a)
+// NS = samples per lane: 8 (256-sample tiles, 128 registers, one CTA per SM) or 4 (128-sample tiles, 64
+// registers, two CTAs = 32 warps per SM: the kernel waits on shared-memory latency and on the block barrier,
+// and twice the resident warps cover both)
+template <bool MULTI, int NS>
+__global__ void __launch_bounds__(32 * IC_WARPS, NS == 8 ? 1 : 2) k_incoherent_v4(const IcArgs a)
 {
+    constexpr int TILE = 32 * NS;                           // output samples per warp
     const int gpc = MULTI ? a.gpc : IC_WARPS, tt = MULTI ? a.tt : 1;
     extern __shared__ float4 ic_smem4[];
     const int rows = a.tw;                                  // input samples staged per chunk: range + 256 tt
     const unsigned tile0 = (unsigned)__cvta_generic_to_shared(ic_smem4), tile_bytes = 128u * (unsigned)rows;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int tbase = blockIdx.x * IC_TILE * tt;
+    const int tbase = blockIdx.x * TILE * tt;
     const int gsel = MULTI ? warp % gpc : warp, sub = MULTI ? warp / gpc : 0;
-    const int t0 = tbase + sub * IC_TILE;
+    const int t0 = tbase + sub * TILE;
     const int grp = blockIdx.y * gpc + gsel;
     const bool live = sub < tt && grp < a.ngroups && t0 < a.nt_out;
     const float *fb = a.fb + (size_t)blockIdx.z * (size_t)a.fb_stride_dm;
 
-    float acc[IC_GROUP][8];
-    float P[IC_MAXSPREAD + 1][8];
+    float acc[IC_GROUP][NS];
+    float P[IC_MAXSPREAD + 1][NS];
 #pragma unroll
     for (int k = 0; k < IC_GROUP; ++k)
 #pragma unroll
-        for (int i = 0; i < 8; ++i) acc[k][i] = 0.f;
+        for (int i = 0; i < NS; ++i) acc[k][i] = 0.f;
 #pragma unroll
     for (int o = 0; o <= IC_MAXSPREAD; ++o)
 #pragma unroll
-        for (int i = 0; i < 8; ++i) P[o][i] = 0.f;
+        for (int i = 0; i < NS; ++i) P[o][i] = 0.f;
 
     int cur = 0, cur_end = 0;
     if (live) {
         cur = a.seg_off[grp];
         cur_end = a.seg_off[grp + 1];
     }
-    uint4 sg = cur < cur_end ? ic_uniform(__ldg(a.segs + cur)) : make_uint4(0x7fffffffu, 0x7fffffffu, 0u, 0u);
+    const uint4 seg_none = make_uint4(0x7fffffffu, 0x7fffffffu, 0u, 0u);
+    uint4 sg = cur < cur_end ? ic_uniform(__ldg(a.segs + cur)) : seg_none;
+    uint4 sg_next = cur + 1 < cur_end ? __ldg(a.segs + cur + 1) : seg_none;   // read one record ahead
 
     // 16-byte pieces of chunk c0 -> buffer `buf`; rows beyond the filterbank and channels beyond nch are zero
     auto stage = [&](int c0, int buf) {
@@ -421,6 +461,8 @@ __global__ void __launch_bounds__(32 * IC_WARPS, 1) k_incoherent_v4(const IcArgs
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
 
+    // Two buffers, two block barriers per chunk.  (Three buffers need only one barrier per chunk -- the copies
+    // of chunk c+1 then go where chunk c-2 was summed from -- but measured slower: c3 47.4 against 46.0 ms.)
     stage(0, 0);
     int buf = 0;
     for (int c0 = 0; c0 < a.nch; c0 += IC4_CC, buf ^= 1) {
@@ -436,14 +478,14 @@ __global__ void __launch_bounds__(32 * IC_WARPS, 1) k_incoherent_v4(const IcArgs
         while ((int)sg.x < c0 + IC4_CC) {
             const int a0 = max((int)sg.x, c0) - c0, a1 = min((int)sg.y, c0 + IC4_CC) - c0;
             const unsigned s0 = sg.z & 0xffffffu, spread = (sg.z >> 24) & 7u;
-            const unsigned r_lane = s0 + lane + sub * IC_TILE;
+            const unsigned r_lane = s0 + lane + sub * TILE;
             const unsigned rowaddr = tile0 + (unsigned)buf * tile_bytes + 128u * r_lane, row7 = r_lane & 7u;
             switch (spread) {
-            case 0: ic4_seg_add<0>(P, rowaddr, row7, a0, a1); break;
-            case 1: ic4_seg_add<1>(P, rowaddr, row7, a0, a1); break;
-            case 2: ic4_seg_add<2>(P, rowaddr, row7, a0, a1); break;
-            case 3: ic4_seg_add<3>(P, rowaddr, row7, a0, a1); break;
-            default: ic4_seg_add<4>(P, rowaddr, row7, a0, a1); break;
+            case 0: ic4_seg_add<0, NS>(P, rowaddr, row7, a0, a1); break;
+            case 1: ic4_seg_add<1, NS>(P, rowaddr, row7, a0, a1); break;
+            case 2: ic4_seg_add<2, NS>(P, rowaddr, row7, a0, a1); break;
+            case 3: ic4_seg_add<3, NS>(P, rowaddr, row7, a0, a1); break;
+            default: ic4_seg_add<4, NS>(P, rowaddr, row7, a0, a1); break;
             }
             if ((int)sg.y > c0 + IC4_CC) break;
             if (sg.z & (1u << 28)) {
@@ -453,28 +495,29 @@ __global__ void __launch_bounds__(32 * IC_WARPS, 1) k_incoherent_v4(const IcArgs
                     if (k > 0) o += (sg.w >> (2 * k)) & 3u;
                     if (o == 0u) {
 #pragma unroll
-                        for (int i = 0; i < 8; ++i) acc[k][i] += P[0][i];
+                        for (int i = 0; i < NS; ++i) acc[k][i] += P[0][i];
                     } else if (o == 1u) {
 #pragma unroll
-                        for (int i = 0; i < 8; ++i) acc[k][i] += P[1][i];
+                        for (int i = 0; i < NS; ++i) acc[k][i] += P[1][i];
                     } else if (o == 2u) {
 #pragma unroll
-                        for (int i = 0; i < 8; ++i) acc[k][i] += P[2][i];
+                        for (int i = 0; i < NS; ++i) acc[k][i] += P[2][i];
                     } else if (o == 3u) {
 #pragma unroll
-                        for (int i = 0; i < 8; ++i) acc[k][i] += P[3][i];
+                        for (int i = 0; i < NS; ++i) acc[k][i] += P[3][i];
                     } else {
 #pragma unroll
-                        for (int i = 0; i < 8; ++i) acc[k][i] += P[4][i];
+                        for (int i = 0; i < NS; ++i) acc[k][i] += P[4][i];
                     }
                 }
 #pragma unroll
                 for (int oo = 0; oo <= IC_MAXSPREAD; ++oo)
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) P[oo][i] = 0.f;
+                    for (int i = 0; i < NS; ++i) P[oo][i] = 0.f;
             }
             ++cur;
-            sg = cur < cur_end ? ic_uniform(__ldg(a.segs + cur)) : make_uint4(0x7fffffffu, 0x7fffffffu, 0u, 0u);
+            sg = ic_uniform(sg_next);
+            sg_next = cur + 1 < cur_end ? __ldg(a.segs + cur + 1) : seg_none;
         }
     }
     if (!live) return;
@@ -485,7 +528,7 @@ __global__ void __launch_bounds__(32 * IC_WARPS, 1) k_incoherent_v4(const IcArgs
         if (k >= gi.y) break;
         float *row = out + (size_t)(gi.x + k) * (size_t)a.ts_pitch;
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
+        for (int i = 0; i < NS; ++i) {
             const int t = t0 + lane + 32 * i;
             if (t < a.nt_out) row[t] = acc[k][i];
         }
@@ -546,8 +589,8 @@ bool incoherent_config(const IncoherentTables &T, int *cc_out, int *tw_out, int 
     }
 }
 
-// k_incoherent_v4: trial groups and time tiles per CTA as above; two tiles of (range + 256 tt) rows of 128 bytes
-static bool incoherent_config_v4(const IncoherentTables &T, int *rows_out, int *gpc_out, int *tt_out, size_t *smem_out)
+// k_incoherent_v4: trial groups and time tiles per CTA as above; two tiles of (range + tile tt) rows of 128 bytes
+static bool incoherent_config_v4(const IncoherentTables &T, int tile, size_t smem_max, int *rows_out, int *gpc_out, int *tt_out, size_t *smem_out)
 {
     const int ngroups = (int)T.groups.size();
     if (ngroups < 1) return false;
@@ -555,9 +598,9 @@ static bool incoherent_config_v4(const IncoherentTables &T, int *rows_out, int *
     if (ny > 65535) return false;
     const int gpc = (ngroups + ny - 1) / ny;
     for (int tt = IC_WARPS / gpc; tt >= 1; --tt) {
-        const int rows = T.range + tt * IC_TILE;
+        const int rows = T.range + tt * tile;
         const size_t smem = 2 * (size_t)rows * 128;
-        if (smem <= (tt > 1 ? 160u : 200u) * 1024) {
+        if (smem <= smem_max) {
             *rows_out = rows; *gpc_out = gpc; *tt_out = tt; *smem_out = smem;
             return true;
         }
@@ -601,19 +644,29 @@ cudaError_t launch_incoherent(const Geometry &g, IncoherentTables &T, const floa
     a.nt_in = (int)nt_in; a.nt_out = (int)nt_out; a.nch = nch; a.ngroups = ngroups;
     size_t smem = 0;
     a.vec_in = (nch % 4 == 0 && fb_stride_dm % 4 == 0 && (reinterpret_cast<uintptr_t>(d_fb) & 15) == 0) ? 1 : 0;
-    // rows readable in 16-byte pieces and two tiles in shared memory: the cp.async / LDS.128 kernel
-    if (a.vec_in && incoherent_config_v4(T, &a.tw, &a.gpc, &a.tt, &smem)) {
-        a.cc = IC4_CC;
-        const bool multi = !(a.gpc == IC_WARPS && a.tt == 1);
-        e = multi ? cudaFuncSetAttribute(k_incoherent_v4<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
-                  : cudaFuncSetAttribute(k_incoherent_v4<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        dim3 grid((unsigned)((nt_out + IC_TILE * a.tt - 1) / (IC_TILE * a.tt)), (unsigned)((ngroups + a.gpc - 1) / a.gpc), (unsigned)g.ndm);
-        if (multi) k_incoherent_v4<true><<<grid, 32 * IC_WARPS, smem, st>>>(a);
-        else k_incoherent_v4<false><<<grid, 32 * IC_WARPS, smem, st>>>(a);
-        e = cudaGetLastError();
-        if (e == cudaSuccess) ++*launches;
-        return e;
+    // rows readable in 16-byte pieces and two tiles in shared memory: the cp.async / LDS.128 kernel, with
+    // 128-sample tiles and two CTAs per SM where two such tiles take at most half of shared memory
+    // (environment CDMT_IC_NS = 8 forces the 256-sample form: c3 48.6 against 41.5 ms, c4 237 / 204, c5 122 / 115;
+    // 64-sample tiles with three CTAs per SM spill at 40 registers: c3 49.8 ms)
+    if (a.vec_in) {
+        static const int force_ns = getenv("CDMT_IC_NS") ? atoi(getenv("CDMT_IC_NS")) : 0;
+        int ns = 0;
+        if (force_ns != 8 && incoherent_config_v4(T, 128, 110u * 1024, &a.tw, &a.gpc, &a.tt, &smem)) ns = 4;
+        else if (incoherent_config_v4(T, 256, 224u * 1024, &a.tw, &a.gpc, &a.tt, &smem)) ns = 8;
+        if (ns) {
+            a.cc = IC4_CC;
+            const bool multi = !(a.gpc == IC_WARPS && a.tt == 1);
+            const void *fn = ns == 4 ? (multi ? (const void *)k_incoherent_v4<true, 4> : (const void *)k_incoherent_v4<false, 4>)
+                                     : (multi ? (const void *)k_incoherent_v4<true, 8> : (const void *)k_incoherent_v4<false, 8>);
+            e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+            const int tile = 32 * ns;
+            dim3 grid((unsigned)((nt_out + tile * a.tt - 1) / (tile * a.tt)), (unsigned)((ngroups + a.gpc - 1) / a.gpc), (unsigned)g.ndm);
+            void *args[] = {&a};
+            e = cudaLaunchKernel(fn, grid, dim3(32 * IC_WARPS), args, smem, st);
+            if (e == cudaSuccess) ++*launches;
+            return e;
+        }
     }
     if (!incoherent_config(T, &a.cc, &a.tw, &a.gpc, &a.tt, &smem)) return cudaErrorInvalidValue;
     const bool multi = !(a.gpc == IC_WARPS && a.tt == 1);

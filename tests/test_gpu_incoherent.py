@@ -3,8 +3,12 @@
   * the shift table (an integer decided in fp64 on both sides) must be identical;
   * on integer-valued filterbanks every partial sum is exact in float32, so the time series must
     match the oracle BIT FOR BIT, whatever the summation order;
-  * on noise-like float data the kernel adds nch float32 numbers in channel order where the oracle
-    adds in double: |delta| <= 2e-5 of the (positive) sums, far inside north_star's 1e-3 of the rms.
+  * on noise-like float data the kernel adds nch float32 numbers (runs of channels that share their
+    shifts first, four channels of a sample pairwise) where the oracle adds in double: |delta| <= 2e-5
+    of the (positive) sums, far inside north_star's 1e-3 of the rms.
+The cases cover the three launch forms: 16-byte rows with 128-sample tiles (two CTAs per SM), the same with
+256-sample tiles (shift range too large for two small tiles), and the general kernel (channel count not a
+multiple of 4, or a shift range beyond what two tiles can hold).
 """
 import numpy as np
 import pytest
@@ -61,7 +65,9 @@ CASES = [
     (36, 16, 16, 2, 600, np.arange(-0.25, 0.2501, 0.002)),                 # c3-like channels (576), time step 1.3 ms
     (3, 2, 1, 1, 2000, np.arange(-0.5, 0.5001, 0.1)),                      # 6 channels (scalar loads), coarse steps
     (7, 4, 2, 3, 1031, np.array([-0.3, -0.299, -0.1, 0.0, 0.004, 0.3])),   # 28 channels, irregular grid
-    (64, 1, 1, 1, 3000, np.arange(0.0, 0.05001, 0.005)),                   # big shifts (range ~520): groups of one trial
+    (64, 1, 1, 1, 3000, np.arange(0.0, 0.05001, 0.005)),                   # big shifts (range ~520): groups of one trial,
+                                                                           # 256-sample tiles of the 16-byte kernel
+    (64, 1, 1, 1, 4000, np.arange(0.0, 0.10001, 0.01)),                    # range ~1040: two tiles do not fit, general kernel
     (10, 8, 8, 1, 300, np.array([0.0])),                                   # single trial = channel sum
 ]
 
