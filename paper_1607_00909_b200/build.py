@@ -7,7 +7,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcdmt.so")
-SOURCES = ["cdmt_kernels.cu", "cdmt_fused.cu", "cdmt_fused2.cu", "cdmt_fused4.cu", "cdmt_fused5.cu", "cdmt_fused6.cu", "cdmt_redigitize.cu", "cdmt_incoherent.cu", "cdmt_api.cu"]
+SOURCES = ["cdmt_kernels.cu", "cdmt_fused.cu", "cdmt_fused2.cu", "cdmt_fused4.cu", "cdmt_fused5.cu", "cdmt_redigitize.cu", "cdmt_incoherent.cu", "cdmt_api.cu"]
 HEADERS = ["cdmt_fft.cuh", "cdmt_fft2.cuh", "cdmt_tmem.cuh", "cdmt_fused_common.cuh", "cdmt_internal.h", os.path.join("..", "..", "include", "cdmt.h")]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "--threads", "4"]

@@ -202,7 +202,7 @@ extern "C" int cdmt_plan_set_option(cdmt_plan *plan, int key, long long value)
         plan->profile = (int)value;
         return CDMT_OK;
     case CDMT_OPT_FUSED_KERNEL:
-        if (value < 0 || value > 6) return CDMT_ERR_ARG;
+        if (value < 0 || value > 5) return CDMT_ERR_ARG;
         plan->force_generic = (int)value;
         return CDMT_OK;
     case CDMT_OPT_HOST_GROUP_BLOCKS:

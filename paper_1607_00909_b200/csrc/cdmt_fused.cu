@@ -433,12 +433,7 @@ cudaError_t launch_fused(const Geometry &g, const Workspace &ws, const float2 *s
     const bool sp_ok = fast_ok && small_phase && fused_sp_supported(M, D, g.hdisc);
     if (force_generic == 5 && !sp_ok) return cudaErrorInvalidValue;
     const bool ws_ok = x2_ok && fused_ws_supported(M, D, g.hdisc, g.nsub, unit0, nunits);
-    if ((force_generic == 4 || force_generic == 6) && !ws_ok) return cudaErrorInvalidValue;
-    if (ws_ok && force_generic == 6) {
-        fa.segsum = reinterpret_cast<double2 *>(d_segsum);
-        if (d_segsum && sums_done) *sums_done = true;
-        return launch_fused_wz(M, logd, fa, h_dm, nunits, st, launches);
-    }
+    if (force_generic == 4 && !ws_ok) return cudaErrorInvalidValue;
     if (force_generic == 3 && !x2_ok) return cudaErrorInvalidValue;
     if (force_generic == 2 && !fast_ok) return cudaErrorInvalidValue;
     // automatic choice: x2 (measured fastest on all five configs: c3 21.8 ms per launch against 22.2 for sp),

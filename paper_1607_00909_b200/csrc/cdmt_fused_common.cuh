@@ -131,11 +131,6 @@ bool fused_ws_supported(int M, int ndec, int hdisc, int nsub, int unit0, int nun
 cudaError_t launch_fused_ws(int M, int logd, const FusedArgs &fa, const double *h_dm, int nunits, cudaStream_t st,
                             long long *launches);
 
-// cdmt_fused6.cu
-bool fused_wz_supported(int M, int ndec, int hdisc, int nsub, int unit0, int nunits);
-cudaError_t launch_fused_wz(int M, int logd, const FusedArgs &fa, const double *h_dm, int nunits, cudaStream_t st,
-                            long long *launches);
-
 // cdmt_fused4.cu
 bool fused_sp_supported(int M, int ndec, int hdisc);
 cudaError_t launch_fused_sp(int M, int logd, const FusedArgs &fa, const double *h_dm, int nunits, cudaStream_t st,

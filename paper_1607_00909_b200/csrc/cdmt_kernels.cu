@@ -8,8 +8,6 @@
 //  k_fused<M, ...>              l.99-103 for a tile of DM trials: chirp on the fly, length-M
 //                               backward FFT, unpad, detect, Stokes I, time integration, pack
 #include "cdmt_fft.cuh"
-#include <cstdlib>
-
 #include "cdmt_internal.h"
 
 namespace cdmt {
@@ -287,98 +285,6 @@ __global__ void __launch_bounds__(L) k_fwd_pass(const void *__restrict__ src_v, 
     }
 }
 
-// The same pass for float32 complex input (pass A with CDMT_IN_CF32, and every pass B), persistent and
-// double-buffered: a CTA walks tiles idx = blockIdx.x, + gridDim.x, ... and copies tile k+1 into the other
-// half of shared memory with 8-byte cp.async while it transforms and stores tile k.  k_fwd_pass is
-// load -> barrier -> transform -> store per CTA with four CTAs per SM, so the memory pipe idles whenever
-// the resident CTAs happen to transform together (pass A 5.2 TB/s, pass B 5.5 TB/s on c3); here every
-// resident CTA always has a tile in flight.
-__device__ __forceinline__ void cp_async8(float2 *dst, const float2 *src)
-{
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
-}
-
-template <int L, int MODE>
-__global__ void __launch_bounds__(L, (L <= 256 ? 3 : L <= 512 ? 2 : 1)) k_fwd_pass_db(const float2 *__restrict__ src_v, float2 *__restrict__ dst,
-                                                   const float2 *__restrict__ tw, const float2 *__restrict__ tw_lo,
-                                                   const float2 *__restrict__ tw_hi, int lo_bits, int nfft, int n1,
-                                                   int n2, int nsub, int step, long long in_stride_pol, int unit0,
-                                                   int ntile, int ntotal)
-{
-    constexpr int NT = L;
-    using Plan = RadixPlan<L>;
-    using Addr = SmemAddr<FWD_BATCH>;
-    using Last = Pass<L, Plan::npass - 1, -1, NT, FWD_BATCH>;
-    constexpr int TILE = L * (FWD_BATCH + 1);   // float2 per buffer: SmemAddr<FWD_BATCH>::size(L)
-    extern __shared__ float2 smem[];
-    const int tid = threadIdx.x;
-
-    auto issue = [&](int idx, float2 *buf) {
-        const int row = idx / ntile, tile = idx - row * ntile;
-        if (MODE == 0) {
-            const int unit = unit0 + (row >> 1), b = unit / nsub, sb = unit % nsub;
-            const float2 *src = src_v + in_row0<0>(sb, row & 1, in_stride_pol) + (size_t)b * step + (size_t)tile * FWD_BATCH;
-#pragma unroll 16
-            for (int e = tid; e < L * FWD_BATCH; e += NT) {
-                const int n1i = e / FWD_BATCH, col = e % FWD_BATCH;
-                cp_async8(buf + Addr::at(n1i, col), src + (size_t)n1i * n2 + col);
-            }
-        } else {
-            const float2 *src = src_v + (size_t)row * nfft + (size_t)tile * FWD_BATCH * n2;
-#pragma unroll 16
-            for (int e = tid; e < L * FWD_BATCH; e += NT) {
-                const int rr = e / L, n2i = e % L;
-                cp_async8(buf + Addr::at(n2i, rr), src + (size_t)rr * n2 + n2i);
-            }
-        }
-        asm volatile("cp.async.commit_group;" ::: "memory");
-    };
-
-    int idx = blockIdx.x, b = 0;
-    if (idx < ntotal) issue(idx, smem);
-    const int nmask = nfft - 1;
-    for (; idx < ntotal; idx += gridDim.x, b ^= 1) {
-        if (idx + (int)gridDim.x < ntotal) {
-            issue(idx + gridDim.x, smem + (b ^ 1) * TILE);
-            asm volatile("cp.async.wait_group 1;" ::: "memory");
-        } else {
-            asm volatile("cp.async.wait_group 0;" ::: "memory");
-        }
-        __syncthreads();
-        float2 v[16];
-        fft_passes<L, 0, -1, NT, FWD_BATCH, false>(v, smem + b * TILE, tw, tid);
-        const int row = idx / ntile, tile = idx - row * ntile;
-        const size_t plane = (size_t)row * nfft;
-#pragma unroll
-        for (int u = 0; u < Last::U; ++u) {
-            const int col = Last::batch_of(tid, u);
-            float2 w = make_float2(1.f, 0.f), ratio = w;
-            if (MODE == 0) {   // four-step twiddles of the outputs k0 + q NS: first term and ratio (see k_fwd_pass)
-                const int n2i = tile * FWD_BATCH + col;
-                const int e0 = (int)(((long long)n2i * Last::out_elem(tid, u, 0)) & nmask);
-                const int es = (int)(((long long)n2i * Last::NS) & nmask);
-                w = cmul(__ldg(tw_hi + (e0 >> lo_bits)), __ldg(tw_lo + (e0 & ((1 << lo_bits) - 1))));
-                ratio = cmul(__ldg(tw_hi + (es >> lo_bits)), __ldg(tw_lo + (es & ((1 << lo_bits) - 1))));
-            }
-#pragma unroll
-            for (int q = 0; q < Last::R; ++q) {
-                const int k = Last::out_elem(tid, u, q);
-                const float2 val = v[u * Last::R + q];
-                if (MODE == 0) {
-                    const int n2i = tile * FWD_BATCH + col;
-                    dst[plane + (size_t)k * n2 + n2i] = cmul(val, w);
-                    if (q + 1 < Last::R) w = cmul(w, ratio);
-                } else {
-                    const int k1 = tile * FWD_BATCH + col;
-                    const int kk = k1 + n1 * k;
-                    dst[plane + ((kk + (nfft >> 1)) & nmask)] = val;
-                }
-            }
-        }
-        __syncthreads();   // this tile's buffer is free for the copies the next iteration issues
-    }
-}
-
 // ------------------------------------------------------------------------------------
 // FP32 FMA rate (roofline denominator)
 // ------------------------------------------------------------------------------------
@@ -506,34 +412,6 @@ static cudaError_t launch_fwd_L(int mode, const Geometry &g, const Workspace &ws
     const int vec16 = (g.in_dtype == 1 || g.in_dtype == 3) && (reinterpret_cast<uintptr_t>(src) & 15) == 0 &&
                       ((long long)in_stride_pol * wb) % 16 == 0 && ((long long)g.step * wb) % 16 == 0 &&
                       ((long long)g.n2 * wb) % 16 == 0;
-    // float32 complex source and two tiles within a third of shared memory: the persistent, double-buffered form
-    static const int fwd_db = getenv("CDMT_FWD_DB") ? atoi(getenv("CDMT_FWD_DB")) : 1;
-    if (fwd_db && (mode == 1 || g.in_dtype == 0) && L >= 64 && 2 * smem <= 75 * 1024) {
-        const int ntile = (mode == 0 ? g.n2 : g.n1) / FWD_BATCH;
-        const long long ntotal = (long long)nunits * 2 * ntile;
-        if (ntotal < (1LL << 31)) {
-            int dev = 0, nsm = 148;
-            cudaGetDevice(&dev);
-            cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-            const int per_sm = (int)((227 * 1024) / (2 * smem + 1024));
-            const long long want = (long long)nsm * (per_sm < 1 ? 1 : per_sm);
-            const unsigned nblk = (unsigned)(ntotal < want ? ntotal : want);
-            if (mode == 0) {
-                e = cudaFuncSetAttribute(k_fwd_pass_db<L, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(2 * smem));
-                if (e != cudaSuccess) return e;
-                k_fwd_pass_db<L, 0><<<nblk, L, 2 * smem, st>>>(reinterpret_cast<const float2 *>(src), dst, tw, ws.tw4_lo, ws.tw4_hi,
-                                                               g.lo_bits, g.nfft, g.n1, g.n2, g.nsub, g.step, in_stride_pol,
-                                                               unit0, ntile, (int)ntotal);
-            } else {
-                e = cudaFuncSetAttribute(k_fwd_pass_db<L, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(2 * smem));
-                if (e != cudaSuccess) return e;
-                k_fwd_pass_db<L, 1><<<nblk, L, 2 * smem, st>>>(reinterpret_cast<const float2 *>(src), dst, tw, ws.tw4_lo, ws.tw4_hi,
-                                                               g.lo_bits, g.nfft, g.n1, g.n2, g.nsub, g.step, in_stride_pol,
-                                                               unit0, ntile, (int)ntotal);
-            }
-            return cudaGetLastError();
-        }
-    }
     if (mode == 0) {
         switch (g.in_dtype) {
         case 0: CDMT_FWD(0, 0); break;

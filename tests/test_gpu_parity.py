@@ -141,8 +141,7 @@ X2_SHAPES = [
 @pytest.mark.parametrize("ref", [synth.REF_CHANNEL, synth.REF_SUBBAND])
 def test_fused_kernel_variants(cdmt, shape, ref):
     """CDMT_OPT_FUSED_KERNEL: software-pipelined packed polarisations (5), warp-specialised packed half
-    transforms with two blocks per CTA (4; 6 = the same with the chirp multiplication in the chirp warps),
-    packed half transforms (3), scalar fast (2) and general (1)."""
+    transforms with two blocks per CTA (4), packed half transforms (3), scalar fast (2) and general (1)."""
     nsub, nsamp, nfft, noverlap, nchan, ndec = shape
     cfg = synth.small_config(nsub=nsub, nsamp=nsamp, nfft=nfft, noverlap=noverlap, nchan=nchan,
                              ndec=ndec, dm=(0.0, 1.5, -3.5, 41.25, 96.0), f_lo=121.0)
@@ -155,7 +154,7 @@ def test_fused_kernel_variants(cdmt, shape, ref):
     if M <= 4096:
         kerns.insert(0, 5)
     if M == 4096 and ndec >= 8:
-        kerns += [4, 6]
+        kerns.append(4)
     for kern in kerns:
         got, _ = gpu_run(cdmt, cfg, x, ref, opts={cdmt.OPT_FUSED_KERNEL: kern})
         worst = check_filterbank(got, want)
@@ -164,9 +163,7 @@ def test_fused_kernel_variants(cdmt, shape, ref):
         # kernel 4 pairs the blocks of a chunk: chunks of three blocks (the third block's CTAs run with the
         # second FFT group idle) with a DM tile that does not divide ndm, and chunks of two blocks (where
         # nblock is odd the last chunk is a lone block, which goes to kernel 3)
-        for opts in ({cdmt.OPT_CHUNK_UNITS: 3 * nsub, cdmt.OPT_DM_TILE: 2}, {cdmt.OPT_CHUNK_UNITS: 2 * nsub},
-                     {cdmt.OPT_FUSED_KERNEL: 6, cdmt.OPT_CHUNK_UNITS: 3 * nsub, cdmt.OPT_DM_TILE: 2},
-                     {cdmt.OPT_FUSED_KERNEL: 6, cdmt.OPT_CHUNK_UNITS: 3 * nsub, cdmt.OPT_DM_TILE: 1}):
+        for opts in ({cdmt.OPT_CHUNK_UNITS: 3 * nsub, cdmt.OPT_DM_TILE: 2}, {cdmt.OPT_CHUNK_UNITS: 2 * nsub}):
             got, _ = gpu_run(cdmt, cfg, x, ref, opts=opts)
             check_filterbank(got, want)
     # a DM tile that does not divide ndm, one unit per chunk
@@ -179,7 +176,7 @@ def test_fused_kernel_choice_is_checked(cdmt):
     """Kernels 2 to 5 refuse shapes they do not cover (status, not a wrong answer)."""
     cfg = synth.small_config(nsub=1, nsamp=2 ** 13, nfft=4096, noverlap=992, nchan=8, ndec=4, dm=(0.0, 3.0))
     x = synth.generate(cfg)
-    for kern in (2, 3, 4, 5, 6):
+    for kern in (2, 3, 4, 5):
         with pytest.raises(cdmt.CdmtError) as e:
             gpu_run(cdmt, cfg, x, opts={cdmt.OPT_FUSED_KERNEL: kern})
         assert e.value.status == cdmt.ERR_CUDA
@@ -389,7 +386,7 @@ def test_errors_are_codes_not_crashes(cdmt):
 
 
 # ---------------------------------------------------------------- repeatability (stands in for racecheck)
-@pytest.mark.parametrize("kern", [4, 6, 3, 5])
+@pytest.mark.parametrize("kern", [4, 3, 5])
 def test_fused_kernels_are_bit_reproducible(cdmt, kern):
     """compute-sanitizer's racecheck is not available on the GPU pool.  The fused kernels exchange data
     through shared memory under split mbarriers; a missing wait would show as run-to-run differences.
