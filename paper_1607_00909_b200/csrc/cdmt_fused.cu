@@ -419,6 +419,7 @@ cudaError_t launch_fused(const Geometry &g, const Workspace &ws, const float2 *s
     fa.dm_first = 0;
     fa.dm_param0 = 0;
     fa.nb_chunk = 0;
+    fa.cta0 = 0;
     fa.segsum = nullptr;
     fa.nblock_total = nblock_total;
     int logd = 0;

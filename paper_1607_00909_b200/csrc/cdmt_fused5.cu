@@ -96,8 +96,9 @@ k_fused_ws(const FusedArgs a, const __grid_constant__ DmParams dmp)
     const int role = warp >> 2;          // 0, 1: FFT group A, B; NGRP: chirp warps
     const int q = warp & 3;              // TMEM lane quadrant
     const int t = tid & (NT - 1);        // thread index inside the role: the same bins in all three
-    const int c = blockIdx.x % a.nchan;
-    const int pl = blockIdx.x / a.nchan; // pair index inside the chunk: (bp, s)
+    const int bx = (int)blockIdx.x + a.cta0;
+    const int c = bx % a.nchan;
+    const int pl = bx / a.nchan;         // pair index inside the chunk: (bp, s)
     const int s = pl % a.nsub, bp = pl / a.nsub;
     const int nb_chunk = a.nb_chunk;     // whole blocks in this chunk (units = nb_chunk * nsub)
     const bool has_b = 2 * bp + 1 < nb_chunk;
@@ -482,6 +483,9 @@ static cudaError_t launch_ws_MD(FusedArgs fa, const double *h_dm, int nunits, cu
     const int ndm_total = fa.ndm;
     fa.nb_chunk = nunits / fa.nsub;
     const int npairs = (fa.nb_chunk + 1) / 2 * fa.nsub;
+    int dev = 0, nsm = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
     for (int d0 = 0; d0 < ndm_total; d0 += DM_PARAM_MAX) {
         const int cnt = ndm_total - d0 < DM_PARAM_MAX ? ndm_total - d0 : DM_PARAM_MAX;
         DmParams dmp;
@@ -490,12 +494,33 @@ static cudaError_t launch_ws_MD(FusedArgs fa, const double *h_dm, int nunits, cu
         fa.dm_first = d0;
         fa.dm_param0 = d0;
         fa.ndm = d0 + cnt;
-        dim3 grid((unsigned)(npairs * fa.nchan), (unsigned)((cnt + fa.dm_tile - 1) / fa.dm_tile));
-        if (sums) k_fused_ws<M, LOGD, true><<<grid, G::NTHREADS, G::smem_bytes, st>>>(fa, dmp);
-        else k_fused_ws<M, LOGD, false><<<grid, G::NTHREADS, G::smem_bytes, st>>>(fa, dmp);
-        e = cudaGetLastError();
+        // Every CTA runs all its trials on one SM for the same time, so a launch of n CTAs on S SMs costs
+        // ceil(n / S) waves: a small launch (a host group of two blocks of c3 is 4608 CTAs = 31.1 waves) idles
+        // through most of its last wave.  Where that matters the CTAs beyond the last full wave are launched
+        // apart, each cut into DM tiles, as many as fill the SMs once: one short wave instead of a long one.
+        const int nctas = npairs * fa.nchan;
+        const int full = nctas / nsm * nsm, rem = nctas - full;
+        const bool split = fa.dm_tile >= cnt && rem > 0 && full > 0 && nctas / nsm < 100 && 2 * rem <= nsm && cnt >= 16;
+        auto launch = [&](int cta0, int n, int tile) {
+            FusedArgs la = fa;
+            la.cta0 = cta0;
+            la.dm_tile = tile;
+            dim3 grid((unsigned)n, (unsigned)((cnt + tile - 1) / tile));
+            if (sums) k_fused_ws<M, LOGD, true><<<grid, G::NTHREADS, G::smem_bytes, st>>>(la, dmp);
+            else k_fused_ws<M, LOGD, false><<<grid, G::NTHREADS, G::smem_bytes, st>>>(la, dmp);
+            ++*launches;
+            return cudaGetLastError();
+        };
+        if (!split) {
+            e = launch(0, nctas, fa.dm_tile);
+        } else {
+            e = launch(0, full, fa.dm_tile);
+            if (e != cudaSuccess) return e;
+            int ny = nsm / rem;
+            if (ny > cnt / 8) ny = cnt / 8;   // at least 8 trials per CTA: its set-up costs about one
+            e = launch(full, rem, (cnt + ny - 1) / ny);
+        }
         if (e != cudaSuccess) return e;
-        ++*launches;
     }
     return cudaSuccess;
 }

@@ -50,6 +50,7 @@ struct FusedArgs {
     int unit0, nsub, nchan, nfft, hdisc, ndec, vdec, ndm, dm_tile, chirp_ref, accurate;
     int dm_first, dm_param0;  // DM range [dm_first, ndm) of this launch; dmp.dm[0] is trial dm_param0
     int nb_chunk;             // k_fused_ws: whole blocks in this chunk (units = nb_chunk * nsub)
+    int cta0;                 // k_fused_ws: blockIdx.x of this launch starts at CTA cta0 of the chunk
     double2 *segsum;          // block sums [ndm][nblock_total][nsub nchan] of (I, I^2) (Alg. 1 l.104), or null
     int nblock_total;         // blocks of this execute (second dimension of segsum)
     double bw_mhz;

@@ -182,7 +182,7 @@ __global__ void __launch_bounds__(256) k_unpack(const void *__restrict__ in, lon
 constexpr int FWD_BATCH = 16;
 
 template <int L, int MODE, int IN>
-__global__ void __launch_bounds__(L, (L == 256 ? ((MODE == 1 || IN == 0 || IN == 2) ? 5 : 4) : 1)) k_fwd_pass(const void *__restrict__ src_v, float2 *__restrict__ dst,
+__global__ void __launch_bounds__(L, (L == 256 ? ((MODE == 1 || IN == 0 || IN == 2) ? 5 : 4) : 0)) k_fwd_pass(const void *__restrict__ src_v, float2 *__restrict__ dst,
                                                 const float2 *__restrict__ tw, const float2 *__restrict__ tw_lo,
                                                 const float2 *__restrict__ tw_hi, int lo_bits, int nfft, int n1,
                                                 int n2, int nsub, int step, long long in_stride_pol, int unit0,
