@@ -116,8 +116,9 @@ k_fused_x2(const FusedArgs a, const __grid_constant__ DmParams dmp)
     uint32_t *tslot = reinterpret_cast<uint32_t *>(barA + 1);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int c = blockIdx.x % a.nchan;
-    const int ulocal = blockIdx.x / a.nchan;
+    const int bx = (int)blockIdx.x + a.cta0;
+    const int c = bx % a.nchan;
+    const int ulocal = bx / a.nchan;
     const int unit = a.unit0 + ulocal, b = unit / a.nsub, s = unit % a.nsub;
 
     if (warp == 0) tmem_alloc<G::TCOLS>(tslot);
@@ -355,6 +356,9 @@ static cudaError_t launch_x2_MD(FusedArgs fa, const double *h_dm, int nunits, cu
     cudaError_t e = cudaFuncSetAttribute(k_fused_x2<M, LOGD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const int ndm_total = fa.ndm;
+    int dev = 0, nsm = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
     for (int d0 = 0; d0 < ndm_total; d0 += DM_PARAM_MAX) {
         const int cnt = ndm_total - d0 < DM_PARAM_MAX ? ndm_total - d0 : DM_PARAM_MAX;
         DmParams dmp;
@@ -363,11 +367,30 @@ static cudaError_t launch_x2_MD(FusedArgs fa, const double *h_dm, int nunits, cu
         fa.dm_first = d0;
         fa.dm_param0 = d0;
         fa.ndm = d0 + cnt;
-        dim3 grid((unsigned)(nunits * fa.nchan), (unsigned)((cnt + fa.dm_tile - 1) / fa.dm_tile));
-        k_fused_x2<M, LOGD><<<grid, M / 32, smem, st>>>(fa, dmp);
-        e = cudaGetLastError();
+        // last wave of a small launch: as in k_fused_ws (cdmt_fused5.cu), the CTAs beyond the last full wave
+        // run as DM tiles that fill the SMs once (c2: 2880 CTAs = 19.5 waves of 148)
+        const int nctas = nunits * fa.nchan, slots = nsm * G::CTAS_PER_SM;
+        const int full = nctas / slots * slots, rem = nctas - full;
+        const bool split = fa.dm_tile >= cnt && rem > 0 && full > 0 && nctas / slots < 100 && 2 * rem <= slots && cnt >= 16;
+        auto launch = [&](int cta0, int n, int tile) {
+            FusedArgs la = fa;
+            la.cta0 = cta0;
+            la.dm_tile = tile;
+            dim3 grid((unsigned)n, (unsigned)((cnt + tile - 1) / tile));
+            k_fused_x2<M, LOGD><<<grid, M / 32, smem, st>>>(la, dmp);
+            ++*launches;
+            return cudaGetLastError();
+        };
+        if (!split) {
+            e = launch(0, nctas, fa.dm_tile);
+        } else {
+            e = launch(0, full, fa.dm_tile);
+            if (e != cudaSuccess) return e;
+            int ny = slots / rem;
+            if (ny > cnt / 8) ny = cnt / 8;
+            e = launch(full, rem, (cnt + ny - 1) / ny);
+        }
         if (e != cudaSuccess) return e;
-        ++*launches;
     }
     return cudaSuccess;
 }
