@@ -31,12 +31,11 @@
 // segment records (one uint4 per ~30 channels) are read from global memory and made warp-uniform by a
 // shuffle.  k_incoherent below is the general form (any channel count and alignment, shift ranges up to
 // ~14 000 samples); k_incoherent_v4 further down is the fast form for filterbanks whose rows can be read
-// in 16-byte pieces.  Measured on c3 (251 fine trials x 96 coherent DMs): 41.5 ms (k_incoherent_v4) against
+// in 16-byte pieces.  Measured on c3 (251 fine trials x 96 coherent DMs): 39.0 ms (k_incoherent_v4) against
 // 54 ms for the per-channel table walk of round 1 and 66 ms for the trial-by-trial kernel before that.
 #include <algorithm>
 #include <cmath>
 #include <cstdint>
-#include <cstdlib>
 #include <cstring>
 
 #include "cdmt_internal.h"
@@ -352,7 +351,8 @@ __global__ void __launch_bounds__(32 * IC_WARPS, 1) k_incoherent(const IcArgs a)
 //  * Everything else -- trial groups, runs, segments, end-of-run hand-over -- as in k_incoherent; the
 //    additions of a run happen in another order (pairs inside a quad first), exact on integer data.
 // ------------------------------------------------------------------------------------------------
-constexpr int IC4_CC = 32;   // channels per chunk = one 128-byte row
+// channels per chunk CC = 32 or 64: one row of the tile is 4 CC bytes (128 or 256); the swizzle acts on the
+// low three bits of the piece number either way (what a quarter warp needs)
 
 __device__ __forceinline__ void ic_cp16(unsigned dst, const void *src, int bytes)
 {
@@ -360,7 +360,7 @@ __device__ __forceinline__ void ic_cp16(unsigned dst, const void *src, int bytes
 }
 
 // P_o[i] += sum of the four channels of quad j at rows s0 + o + lane + 32 i (+ the warp's time tile)
-template <int SP, int NS>
+template <int SP, int NS, int RB>
 __device__ __forceinline__ void ic4_quads(float (&P)[IC_MAXSPREAD + 1][NS], unsigned rowaddr, unsigned row7, int j0, int nq)
 {
 #pragma unroll 1
@@ -368,11 +368,11 @@ __device__ __forceinline__ void ic4_quads(float (&P)[IC_MAXSPREAD + 1][NS], unsi
 #pragma unroll
         for (int o = 0; o <= SP; ++o) {
             // row r = r_lane + o: its swizzle term is ((row7 + o) & 7); 32 i more rows do not change it
-            const unsigned a = rowaddr + 128u * o + ((((unsigned)j ^ (row7 + o)) & 7u) << 4);
+            const unsigned a = rowaddr + (unsigned)RB * o + (((unsigned)j ^ ((row7 + o) & 7u)) << 4);
 #pragma unroll
             for (int i = 0; i < NS; ++i) {
                 float x, y, z, w;
-                asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(x), "=f"(y), "=f"(z), "=f"(w) : "r"(a + 4096u * i));
+                asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(x), "=f"(y), "=f"(z), "=f"(w) : "r"(a + 32u * RB * i));
                 P[o][i] += (x + y) + (z + w);
             }
         }
@@ -380,47 +380,47 @@ __device__ __forceinline__ void ic4_quads(float (&P)[IC_MAXSPREAD + 1][NS], unsi
 }
 // a quad of which only channels [lo, hi) belong to the segment: the same LDS.128, the other components
 // are replaced by zero (lo, hi are warp-uniform, so the selects cost no divergence)
-template <int SP, int NS>
+template <int SP, int NS, int RB>
 __device__ __forceinline__ void ic4_partial(float (&P)[IC_MAXSPREAD + 1][NS], unsigned rowaddr, unsigned row7, int j, int lo, int hi)
 {
     const bool m0 = lo <= 0 && 0 < hi, m1 = lo <= 1 && 1 < hi, m2 = lo <= 2 && 2 < hi, m3 = lo <= 3 && 3 < hi;
 #pragma unroll
     for (int o = 0; o <= SP; ++o) {
-        const unsigned a = rowaddr + 128u * o + ((((unsigned)j ^ (row7 + o)) & 7u) << 4);
+        const unsigned a = rowaddr + (unsigned)RB * o + (((unsigned)j ^ ((row7 + o) & 7u)) << 4);
 #pragma unroll
         for (int i = 0; i < NS; ++i) {
             float x, y, z, w;
-            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(x), "=f"(y), "=f"(z), "=f"(w) : "r"(a + 4096u * i));
+            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(x), "=f"(y), "=f"(z), "=f"(w) : "r"(a + 32u * RB * i));
             P[o][i] += ((m0 ? x : 0.f) + (m1 ? y : 0.f)) + ((m2 ? z : 0.f) + (m3 ? w : 0.f));
         }
     }
 }
 // channels [a0, a1) of the staged chunk (chunk-relative), all with the first shift of `rowaddr`
-template <int SP, int NS>
+template <int SP, int NS, int RB>
 __device__ __forceinline__ void ic4_seg_add(float (&P)[IC_MAXSPREAD + 1][NS], unsigned rowaddr, unsigned row7, int a0, int a1)
 {
     if (a0 & 3) {   // head: the rest of the quad a0 sits in (or the whole segment, if it ends inside that quad)
         const int qe = min((a0 | 3) + 1, a1);
-        ic4_partial<SP, NS>(P, rowaddr, row7, a0 >> 2, a0 & 3, qe - (a0 & ~3));
+        ic4_partial<SP, NS, RB>(P, rowaddr, row7, a0 >> 2, a0 & 3, qe - (a0 & ~3));
         a0 = qe;
     }
     const int nq = (a1 - a0) >> 2;
-    if (nq > 0) ic4_quads<SP, NS>(P, rowaddr, row7, a0 >> 2, nq);
+    if (nq > 0) ic4_quads<SP, NS, RB>(P, rowaddr, row7, a0 >> 2, nq);
     a0 += 4 * nq;
-    if (a0 < a1) ic4_partial<SP, NS>(P, rowaddr, row7, a0 >> 2, 0, a1 - a0);
+    if (a0 < a1) ic4_partial<SP, NS, RB>(P, rowaddr, row7, a0 >> 2, 0, a1 - a0);
 }
 
 // NS = samples per lane: 8 (256-sample tiles, 128 registers, one CTA per SM) or 4 (128-sample tiles, 64
 // registers, two CTAs = 32 warps per SM: the kernel waits on shared-memory latency and on the block barrier,
 // and twice the resident warps cover both)
-template <bool MULTI, int NS>
+template <bool MULTI, int NS, int CC>
 __global__ void __launch_bounds__(32 * IC_WARPS, NS == 8 ? 1 : 2) k_incoherent_v4(const IcArgs a)
 {
     constexpr int TILE = 32 * NS;                           // output samples per warp
     const int gpc = MULTI ? a.gpc : IC_WARPS, tt = MULTI ? a.tt : 1;
     extern __shared__ float4 ic_smem4[];
     const int rows = a.tw;                                  // input samples staged per chunk: range + 256 tt
-    const unsigned tile0 = (unsigned)__cvta_generic_to_shared(ic_smem4), tile_bytes = 128u * (unsigned)rows;
+    const unsigned tile0 = (unsigned)__cvta_generic_to_shared(ic_smem4), tile_bytes = (unsigned)(4 * CC) * (unsigned)rows;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tbase = blockIdx.x * TILE * tt;
     const int gsel = MULTI ? warp % gpc : warp, sub = MULTI ? warp / gpc : 0;
@@ -452,11 +452,11 @@ __global__ void __launch_bounds__(32 * IC_WARPS, NS == 8 ? 1 : 2) k_incoherent_v
     // 16-byte pieces of chunk c0 -> buffer `buf`; rows beyond the filterbank and channels beyond nch are zero
     auto stage = [&](int c0, int buf) {
         const unsigned dst0 = tile0 + (unsigned)buf * tile_bytes;
-        for (int e = tid; e < rows * 8; e += 32 * IC_WARPS) {
-            const int r = e >> 3, j = e & 7, t = tbase + r, c = c0 + 4 * j;
+        for (int e = tid; e < rows * (CC / 4); e += 32 * IC_WARPS) {
+            const int r = e / (CC / 4), j = e % (CC / 4), t = tbase + r, c = c0 + 4 * j;
             const bool ok = t < a.nt_in && c < a.nch;      // nch is a multiple of 4: a quad is in or out
             const float *src = ok ? fb + (size_t)t * a.nch + c : fb;
-            ic_cp16(dst0 + 128u * r + ((unsigned)(j ^ (r & 7)) << 4), src, ok ? 16 : 0);
+            ic_cp16(dst0 + (unsigned)(4 * CC) * r + ((unsigned)(j ^ (r & 7)) << 4), src, ok ? 16 : 0);
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
@@ -465,29 +465,29 @@ __global__ void __launch_bounds__(32 * IC_WARPS, NS == 8 ? 1 : 2) k_incoherent_v
     // of chunk c+1 then go where chunk c-2 was summed from -- but measured slower: c3 47.4 against 46.0 ms.)
     stage(0, 0);
     int buf = 0;
-    for (int c0 = 0; c0 < a.nch; c0 += IC4_CC, buf ^= 1) {
+    for (int c0 = 0; c0 < a.nch; c0 += CC, buf ^= 1) {
         __syncthreads();                                   // the other buffer has been consumed
-        if (c0 + IC4_CC < a.nch) {
-            stage(c0 + IC4_CC, buf ^ 1);
+        if (c0 + CC < a.nch) {
+            stage(c0 + CC, buf ^ 1);
             asm volatile("cp.async.wait_group 1;" ::: "memory");
         } else {
             asm volatile("cp.async.wait_group 0;" ::: "memory");
         }
         __syncthreads();                                   // every thread's pieces of this chunk have landed
         if (!live) continue;
-        while ((int)sg.x < c0 + IC4_CC) {
-            const int a0 = max((int)sg.x, c0) - c0, a1 = min((int)sg.y, c0 + IC4_CC) - c0;
+        while ((int)sg.x < c0 + CC) {
+            const int a0 = max((int)sg.x, c0) - c0, a1 = min((int)sg.y, c0 + CC) - c0;
             const unsigned s0 = sg.z & 0xffffffu, spread = (sg.z >> 24) & 7u;
             const unsigned r_lane = s0 + lane + sub * TILE;
-            const unsigned rowaddr = tile0 + (unsigned)buf * tile_bytes + 128u * r_lane, row7 = r_lane & 7u;
+            const unsigned rowaddr = tile0 + (unsigned)buf * tile_bytes + (unsigned)(4 * CC) * r_lane, row7 = r_lane & 7u;
             switch (spread) {
-            case 0: ic4_seg_add<0, NS>(P, rowaddr, row7, a0, a1); break;
-            case 1: ic4_seg_add<1, NS>(P, rowaddr, row7, a0, a1); break;
-            case 2: ic4_seg_add<2, NS>(P, rowaddr, row7, a0, a1); break;
-            case 3: ic4_seg_add<3, NS>(P, rowaddr, row7, a0, a1); break;
-            default: ic4_seg_add<4, NS>(P, rowaddr, row7, a0, a1); break;
+            case 0: ic4_seg_add<0, NS, 4 * CC>(P, rowaddr, row7, a0, a1); break;
+            case 1: ic4_seg_add<1, NS, 4 * CC>(P, rowaddr, row7, a0, a1); break;
+            case 2: ic4_seg_add<2, NS, 4 * CC>(P, rowaddr, row7, a0, a1); break;
+            case 3: ic4_seg_add<3, NS, 4 * CC>(P, rowaddr, row7, a0, a1); break;
+            default: ic4_seg_add<4, NS, 4 * CC>(P, rowaddr, row7, a0, a1); break;
             }
-            if ((int)sg.y > c0 + IC4_CC) break;
+            if ((int)sg.y > c0 + CC) break;
             if (sg.z & (1u << 28)) {
                 unsigned o = 0;
 #pragma unroll
@@ -590,7 +590,7 @@ bool incoherent_config(const IncoherentTables &T, int *cc_out, int *tw_out, int 
 }
 
 // k_incoherent_v4: trial groups and time tiles per CTA as above; two tiles of (range + tile tt) rows of 128 bytes
-static bool incoherent_config_v4(const IncoherentTables &T, int tile, size_t smem_max, int *rows_out, int *gpc_out, int *tt_out, size_t *smem_out)
+static bool incoherent_config_v4(const IncoherentTables &T, int tile, int cc, size_t smem_max, int *rows_out, int *gpc_out, int *tt_out, size_t *smem_out)
 {
     const int ngroups = (int)T.groups.size();
     if (ngroups < 1) return false;
@@ -599,7 +599,7 @@ static bool incoherent_config_v4(const IncoherentTables &T, int tile, size_t sme
     const int gpc = (ngroups + ny - 1) / ny;
     for (int tt = IC_WARPS / gpc; tt >= 1; --tt) {
         const int rows = T.range + tt * tile;
-        const size_t smem = 2 * (size_t)rows * 128;
+        const size_t smem = 2 * (size_t)rows * 4 * cc;
         if (smem <= smem_max) {
             *rows_out = rows; *gpc_out = gpc; *tt_out = tt; *smem_out = smem;
             return true;
@@ -646,18 +646,27 @@ cudaError_t launch_incoherent(const Geometry &g, IncoherentTables &T, const floa
     a.vec_in = (nch % 4 == 0 && fb_stride_dm % 4 == 0 && (reinterpret_cast<uintptr_t>(d_fb) & 15) == 0) ? 1 : 0;
     // rows readable in 16-byte pieces and two tiles in shared memory: the cp.async / LDS.128 kernel, with
     // 128-sample tiles and two CTAs per SM where two such tiles take at most half of shared memory
-    // (environment CDMT_IC_NS = 8 forces the 256-sample form: c3 48.6 against 41.5 ms, c4 237 / 204, c5 122 / 115;
-    // 64-sample tiles with three CTAs per SM spill at 40 registers: c3 49.8 ms)
+    // (the 256-sample form where both apply: c3 48.6 against 41.5 ms, c4 237 / 204, c5 122 / 115; 64-sample
+    // tiles with three CTAs per SM spill at 40 registers: c3 49.8 ms)
     if (a.vec_in) {
-        static const int force_ns = getenv("CDMT_IC_NS") ? atoi(getenv("CDMT_IC_NS")) : 0;
-        int ns = 0;
-        if (force_ns != 8 && incoherent_config_v4(T, 128, 110u * 1024, &a.tw, &a.gpc, &a.tt, &smem)) ns = 4;
-        else if (incoherent_config_v4(T, 256, 224u * 1024, &a.tw, &a.gpc, &a.tt, &smem)) ns = 8;
+        // 64 channels per chunk halve the block barriers per channel (c3 41.5 -> 39.0 ms, c4 204 -> 162 ms) unless
+        // the larger tiles leave room for fewer time tiles per CTA (c5: 7 trial groups x 2 time tiles only with 32)
+        int ns = 0, cc = 0;
+        {
+            int tw64 = 0, gpc64 = 0, tt64 = 0, tw32 = 0, gpc32 = 0, tt32 = 0;
+            size_t sm64 = 0, sm32 = 0;
+            const bool ok64 = incoherent_config_v4(T, 128, 64, 110u * 1024, &tw64, &gpc64, &tt64, &sm64);
+            const bool ok32 = incoherent_config_v4(T, 128, 32, 110u * 1024, &tw32, &gpc32, &tt32, &sm32);
+            if (ok64 && (!ok32 || tt64 >= tt32)) ns = 4, cc = 64, a.tw = tw64, a.gpc = gpc64, a.tt = tt64, smem = sm64;
+            else if (ok32) ns = 4, cc = 32, a.tw = tw32, a.gpc = gpc32, a.tt = tt32, smem = sm32;
+            else if (incoherent_config_v4(T, 256, 32, 224u * 1024, &a.tw, &a.gpc, &a.tt, &smem)) ns = 8, cc = 32;
+        }
         if (ns) {
-            a.cc = IC4_CC;
+            a.cc = cc;
             const bool multi = !(a.gpc == IC_WARPS && a.tt == 1);
-            const void *fn = ns == 4 ? (multi ? (const void *)k_incoherent_v4<true, 4> : (const void *)k_incoherent_v4<false, 4>)
-                                     : (multi ? (const void *)k_incoherent_v4<true, 8> : (const void *)k_incoherent_v4<false, 8>);
+            const void *fn = ns == 8 ? (multi ? (const void *)k_incoherent_v4<true, 8, 32> : (const void *)k_incoherent_v4<false, 8, 32>)
+                           : cc == 64 ? (multi ? (const void *)k_incoherent_v4<true, 4, 64> : (const void *)k_incoherent_v4<false, 4, 64>)
+                                      : (multi ? (const void *)k_incoherent_v4<true, 4, 32> : (const void *)k_incoherent_v4<false, 4, 32>);
             e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
             if (e != cudaSuccess) return e;
             const int tile = 32 * ns;
