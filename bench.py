@@ -75,6 +75,14 @@ def rank_piece(cfg: synth.Config, rank: int, world: int, shard: str):
         if s1 <= s0:
             raise SystemExit("--shard subband needs at least one subband per rank")
         return dataclasses.replace(cfg, nsub=s1 - s0, fcen_mhz=cfg.fcen_mhz[s0:s1]), s0
+    if shard == "dm" and world > 1:
+        # few subbands -> split the DM trials; every rank repeats the forward FFT (a1-a3)
+        # of the whole observation and runs the DM loop over its own contiguous range of trials
+        import dataclasses
+        d0, d1 = subband_range(cfg.ndm, rank, world)
+        if d1 <= d0:
+            raise SystemExit("--shard dm needs at least one DM trial per rank")
+        return dataclasses.replace(cfg, dm=cfg.dm[d0:d1]), 0
     return rank_workload(cfg, rank, world), 0
 
 
@@ -265,8 +273,9 @@ def workload_config(cfg, args):
                cfg.ndm, "int8" if cfg.in_dtype == synth.IN_CI8 else "complex64"),
             "nsub": cfg.nsub, "nsamp": cfg.nsamp, "nfft": cfg.nfft, "noverlap": cfg.noverlap,
             "nchan": cfg.nchan, "ndec": cfg.ndec, "ndm": cfg.ndm, "nblock": cfg.nblock,
-            "parallelism": ("subbands of one observation split over %d GPUs (no collective)" % args.gpus)
-                           if getattr(args, "shard", "replicas") == "subband" and args.gpus > 1 else
+            "parallelism": ("%s of one observation split over %d GPUs (no collective)" % (
+                                {"subband": "subbands", "dm": "DM trials"}[args.shard], args.gpus))
+                           if getattr(args, "shard", "replicas") in ("subband", "dm") and args.gpus > 1 else
                            "replicas x%d (one observation per GPU, no collective)" % args.gpus,
             "l2": "inputs (%.1f GB) and spectra exceed the 126 MB L2; no flush needed" % (
                 cfg.nsub * 2 * cfg.nsamp * (2 if cfg.in_dtype == synth.IN_CI8 else 8) / 1e9)}
@@ -287,9 +296,11 @@ def main():
     ap.add_argument("--gen-threads", type=int, default=0)
     ap.add_argument("--host-group-blocks", type=int, default=0,
                     help="CDMT_OPT_HOST_GROUP_BLOCKS of the end-to-end leg (0 = library default)")
-    ap.add_argument("--shard", default="replicas", choices=["replicas", "subband"],
-                    help="N > 1: one observation per GPU (weak scaling, default) or the subbands of one "
-                         "observation split over the GPUs (strong scaling); neither has a collective")
+    ap.add_argument("--shard", default="replicas", choices=["replicas", "subband", "dm"],
+                    help="N > 1: one observation per GPU (weak scaling, default), or ONE observation with its "
+                         "subbands (output channels concatenate) or its DM trials (output planes concatenate; the "
+                         "forward FFT is repeated on every rank) split over the GPUs (strong scaling); none has a "
+                         "collective")
     ap.add_argument("--no-redigitize", action="store_true", help="skip the extra cdmt_redigitize timing (N1)")
     ap.add_argument("--no-incoherent", action="store_true", help="skip the extra cdmt_incoherent_dedisperse timing (N2)")
     ap.add_argument("--fine-step", type=float, default=0.002, help="fine DM step of the incoherent leg (PAPER.md:141)")
@@ -310,7 +321,7 @@ def main():
         return
     cfg, sub0 = rank_piece(full_cfg, rank, world, args.shard)
     gen_cfg = full_cfg if args.shard == "subband" and world > 1 else cfg   # generator sees global subband indices
-    strong = args.shard == "subband" and world > 1
+    strong = args.shard in ("subband", "dm") and world > 1
 
     import torch
     import torch.distributed as dist

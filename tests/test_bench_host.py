@@ -111,3 +111,19 @@ def test_subband_sharding_partitions_the_observation():
     pc, s0 = bench.rank_piece(small, 1, 2, "subband")
     got = np.stack([synth.generate_subband(small, s0 + s) for s in range(pc.nsub)])
     assert np.array_equal(got, whole[2:4])
+
+
+def test_dm_sharding_partitions_the_trials():
+    """--shard dm (few subbands -> split the DM trials): the ranks' DM ranges tile the
+    list without overlap; every rank keeps all subbands, blocks and the seed of the one observation."""
+    c2 = synth.make_config("c2")
+    got = []
+    for r in range(3):
+        piece, s0 = bench.rank_piece(synth.make_config("c2"), r, 3, "dm")
+        assert s0 == 0 and piece.nsub == c2.nsub and piece.nblock == c2.nblock and piece.seed == c2.seed
+        assert np.array_equal(piece.fcen_mhz, c2.fcen_mhz)
+        got.append(piece.dm)
+    assert np.array_equal(np.concatenate(got), c2.dm)
+    assert max(len(g) for g in got) - min(len(g) for g in got) <= 1
+    # the whole-job metric counts the observation once
+    assert bench.whole_job_value(c2, 1, 0.01) == c2.nsub * c2.nsamp * c2.ndm / 0.01
