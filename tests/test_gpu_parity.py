@@ -358,6 +358,9 @@ def test_subband_shards_concatenate_to_the_unsharded_filterbank(cdmt):
             parts.append(got)
         # output channels descend in frequency: the highest subbands come first
         assert np.array_equal(np.concatenate(parts[::-1], axis=2), whole), world
+    # --shard dm: contiguous ranges of the DM trials; the DM planes concatenate
+    parts = [gpu_run(cdmt, bench.rank_piece(cfg, rank, 2, "dm")[0], x)[0] for rank in range(2)]
+    assert np.array_equal(np.concatenate(parts, axis=0), whole)
 
 
 def test_errors_are_codes_not_crashes(cdmt):
