@@ -583,6 +583,10 @@ def main():
                      "bound": "alu", "achieved_tadd_s": adds_done / ims / 1e9, "peak_tadd_s": peak_add,
                      "frac": adds_done / ims / 1e9 / peak_add,
                      "definition_tadd_s": adds_def / ims / 1e9,
+                     # every addition into a run sum reads one 4-byte word from shared memory: 32 words per
+                     # clock and SM; the time those reads alone take (the bound of this formulation)
+                     "smem_floor_ms": adds_done * 4.0 / 128.0 / (148 * 1.965e9) * 1e3,
+                     "frac_of_smem_floor": adds_done * 4.0 / 128.0 / (148 * 1.965e9) * 1e3 / ims,
                      "peak_source": "derived: 148 SM x 128 FP32 lanes x 1.965 GHz (one FADD per lane and clock)",
                      "out_bytes": int(d_ts.numel() * 4), "semicoherent_step_ms": step_ms,
                      "note": "cdmt_incoherent_dedisperse (+ cdmt_incoherent_carry) on every block group of the step, "
