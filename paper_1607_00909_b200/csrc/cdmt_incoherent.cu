@@ -336,7 +336,7 @@ __global__ void __launch_bounds__(32 * IC_WARPS, 1) k_incoherent(const IcArgs a)
 // k_incoherent_v4: the same sums for filterbanks whose rows can be read in 16-byte pieces (channel count
 // a multiple of 4, aligned planes) and whose shift range lets two tiles fit shared memory.
 //
-//  * The tile keeps the filterbank's own order, [time][32 channels] = 128-byte rows, and is filled by
+//  * The tile keeps the filterbank's own order, [time][CC channels] (CC = 32 or 64: 128- or 256-byte rows), and is filled by
 //    16-byte cp.async copies (no registers, no transposing stores) into one of TWO buffers: the copies of
 //    chunk c+1 fly while chunk c is summed.  (One CTA of 16 warps x 128 registers fills an SM, so in
 //    k_incoherent the global loads of a chunk -- two batches, ~1.5 us each -- are exposed once per chunk,
@@ -350,9 +350,9 @@ __global__ void __launch_bounds__(32 * IC_WARPS, 1) k_incoherent(const IcArgs a)
 //    zeros (single LDS.32 column reads would meet 4-way bank conflicts in this layout).
 //  * Everything else -- trial groups, runs, segments, end-of-run hand-over -- as in k_incoherent; the
 //    additions of a run happen in another order (pairs inside a quad first), exact on integer data.
+//  * The swizzle acts on the low three bits of the piece number for either row length (what a quarter
+//    warp needs); 64 channels per chunk halve the block barriers per channel.
 // ------------------------------------------------------------------------------------------------
-// channels per chunk CC = 32 or 64: one row of the tile is 4 CC bytes (128 or 256); the swizzle acts on the
-// low three bits of the piece number either way (what a quarter warp needs)
 
 __device__ __forceinline__ void ic_cp16(unsigned dst, const void *src, int bytes)
 {

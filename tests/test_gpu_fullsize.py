@@ -284,3 +284,50 @@ def test_subband_reference_mode_c2_sample(cdmt):
     blocks = np.stack([keep[s][:, b * cfg.step:b * cfg.step + cfg.nfft] for s, b in units])
     ref = orc.units(orc.Params(**cfg.plan_kwargs(synth.REF_SUBBAND)), [s for s, _ in units], blocks)
     compare_units(cfg, got_units, list(ref))
+
+
+@pytest.mark.parametrize("name", ["c3", "c4"])
+def test_every_unit_of_a_config_when_asked(cdmt, name):
+    """Opt-in (CDMT_FULL_PARITY=c3,c4; about 11 / 13 minutes of oracle time on 16 host cores): EVERY
+    (subband, block) unit of the config -- not a sample -- against the oracle, subband by subband, all DM
+    trials, at north_star's 1e-3 x rms (rms over the subband's units of that trial), with the peak
+    positions of every clear maximum.  The result of the round's run is recorded in DESIGN.md section 3."""
+    import os
+    from concurrent.futures import ThreadPoolExecutor
+    if name not in os.environ.get("CDMT_FULL_PARITY", "").split(","):
+        pytest.skip("set CDMT_FULL_PARITY=%s to run" % name)
+    cfg = synth.make_config(name)
+    d_in, _ = upload(cfg, subbands=[])
+    plan = cdmt.cdmt_plan_create(**cfg.plan_kwargs())
+    q = cdmt.cdmt_plan_query(plan, cfg.nsamp)
+    nt, nch = q["nout_per_chan"], cfg.nsub * cfg.nchan
+    out = nan_filled((cfg.ndm, nt, nch))
+    ws = torch.empty(q["workspace_bytes"], dtype=torch.uint8, device="cuda")
+    cdmt.cdmt_execute(plan, d_in, cfg.nsamp, cfg.nsamp, out, nt * nch, ws, ws.numel())
+    torch.cuda.synchronize()
+    assert_all_written(out)
+    del d_in, ws
+    p = orc.Params(**cfg.plan_kwargs())
+    worst, nunits, npeaks = 0.0, 0, 0
+    with ThreadPoolExecutor(2) as ex:
+        nxt = ex.submit(synth.generate_subband, cfg, 0)
+        for s in range(cfg.nsub):
+            xs = nxt.result()
+            if s + 1 < cfg.nsub:
+                nxt = ex.submit(synth.generate_subband, cfg, s + 1)
+            blocks = np.stack([xs[:, b * cfg.step:b * cfg.step + cfg.nfft] for b in range(cfg.nblock)])
+            ref = np.stack(list(orc.units(p, [s] * cfg.nblock, blocks)))           # [block][dm][q][c]
+            got = np.stack([gpu_unit_slice(out, cfg, s, b) for b in range(cfg.nblock)]).astype(np.float64)
+            rms = np.sqrt(np.mean(ref ** 2, axis=(0, 2, 3)))                       # per DM trial
+            err = np.abs(got - ref).max(axis=(0, 2, 3))
+            assert (err <= TOL * rms).all(), (s, float((err / rms).max()))
+            worst = max(worst, float((err / rms).max()))
+            g, r = got.sum(-1), ref.sum(-1)                                        # [block][dm][q]
+            top = np.sort(r, axis=2)
+            clear = top[..., -1] - top[..., -2] > 2e-3 * np.sqrt(np.mean(r ** 2, axis=2))
+            assert np.array_equal(g.argmax(axis=2)[clear], r.argmax(axis=2)[clear]), s
+            npeaks += int(clear.sum())
+            nunits += cfg.nblock
+    assert nunits == cfg.nsub * cfg.nblock
+    print("\n%s: all %d units x %d DM trials: max |delta| / rms = %.3g; %d peak positions equal" % (
+        name, nunits, cfg.ndm, worst, npeaks))
