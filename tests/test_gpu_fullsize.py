@@ -286,12 +286,13 @@ def test_subband_reference_mode_c2_sample(cdmt):
     compare_units(cfg, got_units, list(ref))
 
 
-@pytest.mark.parametrize("name", ["c3", "c4"])
+@pytest.mark.parametrize("name", ["c3", "c4", "c5"])
 def test_every_unit_of_a_config_when_asked(cdmt, name):
-    """Opt-in (CDMT_FULL_PARITY=c3,c4; about 11 / 13 minutes of oracle time on 16 host cores): EVERY
-    (subband, block) unit of the config -- not a sample -- against the oracle, subband by subband, all DM
-    trials, at north_star's 1e-3 x rms (rms over the subband's units of that trial), with the peak
-    positions of every clear maximum.  The result of the round's run is recorded in DESIGN.md section 3."""
+    """Opt-in (CDMT_FULL_PARITY=c3,c4,c5; about 11 / 13 / 80 minutes of oracle time on 16 host cores): EVERY
+    (subband, block) unit of the config -- not a sample -- against the oracle, subband by subband in runs of
+    up to 42 blocks, all DM trials, at north_star's 1e-3 x rms (rms over the run's units of that trial),
+    with the peak positions of every clear maximum.  The whole filterbank set is resident (c5: 136 GB).
+    The results of the round's runs are recorded in DESIGN.md section 3 and profiles/r2_full_parity.md."""
     import os
     from concurrent.futures import ThreadPoolExecutor
     if name not in os.environ.get("CDMT_FULL_PARITY", "").split(","):
@@ -315,19 +316,21 @@ def test_every_unit_of_a_config_when_asked(cdmt, name):
             xs = nxt.result()
             if s + 1 < cfg.nsub:
                 nxt = ex.submit(synth.generate_subband, cfg, s + 1)
-            blocks = np.stack([xs[:, b * cfg.step:b * cfg.step + cfg.nfft] for b in range(cfg.nblock)])
-            ref = np.stack(list(orc.units(p, [s] * cfg.nblock, blocks)))           # [block][dm][q][c]
-            got = np.stack([gpu_unit_slice(out, cfg, s, b) for b in range(cfg.nblock)]).astype(np.float64)
-            rms = np.sqrt(np.mean(ref ** 2, axis=(0, 2, 3)))                       # per DM trial
-            err = np.abs(got - ref).max(axis=(0, 2, 3))
-            assert (err <= TOL * rms).all(), (s, float((err / rms).max()))
-            worst = max(worst, float((err / rms).max()))
-            g, r = got.sum(-1), ref.sum(-1)                                        # [block][dm][q]
-            top = np.sort(r, axis=2)
-            clear = top[..., -1] - top[..., -2] > 2e-3 * np.sqrt(np.mean(r ** 2, axis=2))
-            assert np.array_equal(g.argmax(axis=2)[clear], r.argmax(axis=2)[clear]), s
-            npeaks += int(clear.sum())
-            nunits += cfg.nblock
+            for b0 in range(0, cfg.nblock, 42):
+                bs = range(b0, min(cfg.nblock, b0 + 42))
+                blocks = np.stack([xs[:, b * cfg.step:b * cfg.step + cfg.nfft] for b in bs])
+                ref = np.stack(list(orc.units(p, [s] * len(bs), blocks)))          # [block][dm][q][c]
+                got = np.stack([gpu_unit_slice(out, cfg, s, b) for b in bs]).astype(np.float64)
+                rms = np.sqrt(np.mean(ref ** 2, axis=(0, 2, 3)))                   # per DM trial
+                err = np.abs(got - ref).max(axis=(0, 2, 3))
+                assert (err <= TOL * rms).all(), (s, b0, float((err / rms).max()))
+                worst = max(worst, float((err / rms).max()))
+                g, r = got.sum(-1), ref.sum(-1)                                    # [block][dm][q]
+                top = np.sort(r, axis=2)
+                clear = top[..., -1] - top[..., -2] > 2e-3 * np.sqrt(np.mean(r ** 2, axis=2))
+                assert np.array_equal(g.argmax(axis=2)[clear], r.argmax(axis=2)[clear]), (s, b0)
+                npeaks += int(clear.sum())
+                nunits += len(bs)
     assert nunits == cfg.nsub * cfg.nblock
     print("\n%s: all %d units x %d DM trials: max |delta| / rms = %.3g; %d peak positions equal" % (
         name, nunits, cfg.ndm, worst, npeaks))
