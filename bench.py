@@ -2,13 +2,18 @@
 """bench.py -- throughput of the cdmt hot path on B200 (contract: see DESIGN.md "Measurement").
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config c3] [--impl ours|reference]
+                  [--shard replicas|subband|dm] [--survey]
 
 A "step" is one pass of the whole hot path (unpack + forward FFT + fused per-DM kernel, every
 block, every DM) over one synthetic observation of the named config.  Metric (BASELINE.json):
-input samples x DM trials per second = nsub * T * ndm / t.  One JSON line is printed by rank 0.
+input samples x DM trials per second = nsub * T * ndm / t.  One JSON line is printed by rank 0:
+`value` from device-resident input, `e2e` / `e2e_8bit_output` through cdmt_execute_host_async with
+pinned host buffers, `roofline` of the fused per-DM kernel, the extra legs `redigitize` (8-bit output,
+Alg. 1 l.104-106) and `incoherent` (semi-coherent search), `cpu_baseline` (the oracle).
 
-N > 1 (torchrun): the path has no exchange step, so each rank runs its own observation of the
-same config (another beam: other seed) on its own GPU -- weak scaling, no data-path collective;
+N > 1 (torchrun): the path has no exchange step, so by default each rank runs its own observation of
+the same config (another beam: other seed) on its own GPU -- weak scaling, no data-path collective;
+--shard subband / dm split ONE observation over the ranks instead (strong scaling, still no collective).
 torch.distributed is used for the barrier and the max-over-ranks of the device time only.
 """
 from __future__ import annotations
