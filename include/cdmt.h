@@ -243,6 +243,25 @@ int cdmt_redigitize(cdmt_plan *plan, const float *d_fb, long long fb_stride_dm, 
                     float *d_offset, float *d_scale, void *d_workspace, size_t workspace_bytes,
                     void *cuda_stream);
 int cdmt_redigitize_workspace_bytes(const cdmt_plan *plan, long long nblock, size_t *workspace_bytes);
+/*
+ * cdmt_redigitize for callers that cannot allocate device memory (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): same arguments, results and kernels, but no
+ * workspace -- the block sums go to a fixed scratch array inside the library (a file-scope device array
+ * of cdmt_redigitize_static_max_bytes() = 4 MiB, which every GPU that loads the library holds until
+ * the process exits).  The call allocates nothing (no cudaMalloc / cudaFree / pinned memory).
+ *   Limit: ndm * nblock * nsub*nchan * 16 bytes <= 4 MiB, i.e. at most 262144 (DM, block, channel)
+ *   triples per call; a larger batch returns CDMT_ERR_WORKSPACE ("workspace too small") before anything
+ *   is launched -- split it into groups of blocks, or use cdmt_redigitize with your own workspace.
+ *   Sharing: all calls on a device use the one array.  Nothing in it needs to start at zero (the first
+ *   kernel overwrites every entry the second reads), but two calls that overlap on the GPU -- other
+ *   streams, other plans, other host threads -- race on it: order them on one stream or with events.
+ *   The array's device address is looked up once per device, with the caller's current device.
+ * Errors: as cdmt_redigitize, without the workspace-pointer checks.
+ */
+int cdmt_redigitize_static(cdmt_plan *plan, const float *d_fb, long long fb_stride_dm, long long nblock,
+                           double qmean, double qstd, unsigned char *d_codes, long long codes_stride_dm,
+                           float *d_offset, float *d_scale, void *cuda_stream);
+int cdmt_redigitize_static_max_bytes(size_t *max_bytes);
 /* Alg. 1 l.105-106 only, from block sums already taken (cdmt_execute_sums): reads the filterbank once
  * (4 bytes read, 1 byte written per sample).  d_segsum as in cdmt_execute_sums; two kernels. */
 int cdmt_redigitize_sums(cdmt_plan *plan, const float *d_fb, long long fb_stride_dm, long long nblock,

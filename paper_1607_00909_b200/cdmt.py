@@ -30,6 +30,7 @@ EXPORTS = [
     "cdmt_execute", "cdmt_execute_sums", "cdmt_execute_host", "cdmt_execute_host_async", "cdmt_host_layout",
     "cdmt_host_scratch_bytes", "cdmt_host_traffic_bytes", "cdmt_unpack",
     "cdmt_forward_spectrum", "cdmt_redigitize", "cdmt_redigitize_sums", "cdmt_redigitize_workspace_bytes",
+    "cdmt_redigitize_static", "cdmt_redigitize_static_max_bytes",
     "cdmt_incoherent_query", "cdmt_incoherent_shifts", "cdmt_incoherent_dedisperse", "cdmt_incoherent_carry", "cdmt_incoherent_work",
     "cdmt_sweep_seconds", "cdmt_min_overlap", "cdmt_suggest_sizes",
     "cdmt_multiplan_create", "cdmt_multiplan_destroy", "cdmt_multiplan_query", "cdmt_multiplan_group",
@@ -65,6 +66,8 @@ _lib.cdmt_unpack.argtypes = [_vp, _vp, _ll, _ll, _vp, _vp]
 _lib.cdmt_forward_spectrum.argtypes = [_vp, _vp, _ll, _ll, _vp, _vp, _sz, _vp]
 _lib.cdmt_redigitize.argtypes = [_vp, _vp, _ll, _ll, _d, _d, _vp, _ll, _vp, _vp, _vp, _sz, _vp]
 _lib.cdmt_redigitize_workspace_bytes.argtypes = [_vp, _ll, C.POINTER(_sz)]
+_lib.cdmt_redigitize_static.argtypes = [_vp, _vp, _ll, _ll, _d, _d, _vp, _ll, _vp, _vp, _vp]
+_lib.cdmt_redigitize_static_max_bytes.argtypes = [C.POINTER(_sz)]
 _lib.cdmt_incoherent_query.argtypes = [_vp, _i, C.POINTER(_d), _ll, C.POINTER(_i), C.POINTER(_i), C.POINTER(_ll),
                                        C.POINTER(_i), C.POINTER(_sz)]
 _lib.cdmt_incoherent_shifts.argtypes = [_vp, _i, C.POINTER(_d), _vp]
@@ -259,6 +262,20 @@ def cdmt_redigitize(plan: Plan, d_fb, fb_stride_dm: int, nblock: int, qmean: flo
                               _ptr(d_codes), int(codes_stride_dm), _ptr(d_offset), _ptr(d_scale),
                               _ptr(d_workspace), int(workspace_bytes), _stream(stream))
     _check(st, "cdmt_redigitize")
+
+
+def cdmt_redigitize_static(plan: Plan, d_fb, fb_stride_dm: int, nblock: int, qmean: float, qstd: float, d_codes,
+                           codes_stride_dm: int, d_offset, d_scale, stream=None):
+    st = _lib.cdmt_redigitize_static(plan.handle, _ptr(d_fb), int(fb_stride_dm), int(nblock), float(qmean),
+                                     float(qstd), _ptr(d_codes), int(codes_stride_dm), _ptr(d_offset),
+                                     _ptr(d_scale), _stream(stream))
+    _check(st, "cdmt_redigitize_static")
+
+
+def cdmt_redigitize_static_max_bytes() -> int:
+    n = _sz(0)
+    _check(_lib.cdmt_redigitize_static_max_bytes(C.byref(n)), "cdmt_redigitize_static_max_bytes")
+    return int(n.value)
 
 
 def cdmt_redigitize_sums(plan: Plan, d_fb, fb_stride_dm: int, nblock: int, qmean: float, qstd: float, d_segsum,

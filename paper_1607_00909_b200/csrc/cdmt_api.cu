@@ -722,6 +722,37 @@ extern "C" int cdmt_redigitize(cdmt_plan *plan, const float *d_fb, long long fb_
                                         &plan->last_launches));
 }
 
+// cdmt_redigitize without a caller-supplied workspace and without any allocation: the block sums live in a
+// file-scope device array of the library (cdmt_redigitize.cu) of cdmt_redigitize_static_max_bytes() bytes.
+extern "C" int cdmt_redigitize_static_max_bytes(size_t *max_bytes)
+{
+    if (!max_bytes) return CDMT_ERR_ARG;
+    *max_bytes = redigitize_static_max_bytes();
+    return CDMT_OK;
+}
+
+extern "C" int cdmt_redigitize_static(cdmt_plan *plan, const float *d_fb, long long fb_stride_dm, long long nblock,
+                                      double qmean, double qstd, unsigned char *d_codes, long long codes_stride_dm,
+                                      float *d_offset, float *d_scale, void *cuda_stream)
+{
+    if (!plan || !d_fb || !d_codes || !d_offset || !d_scale) return CDMT_ERR_ARG;
+    if (!(qstd > 0.0) || !std::isfinite(qstd) || !std::isfinite(qmean)) return CDMT_ERR_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_fb) & 3) != 0 || (reinterpret_cast<uintptr_t>(d_offset) & 3) != 0 ||
+        (reinterpret_cast<uintptr_t>(d_scale) & 3) != 0)
+        return CDMT_ERR_ARG;
+    const Geometry &g = plan->g;
+    if (nblock < 1 || nblock > 65535 || g.ndm > 65535) return CDMT_ERR_SIZE;
+    const long long plane = nblock * g.vdec * (long long)g.nsub * g.nchan;
+    if (fb_stride_dm < plane || codes_stride_dm < plane) return CDMT_ERR_SIZE;
+    if (nblock * g.vdec > 65535LL * 16) return CDMT_ERR_SIZE;
+    // the block sums of this batch must fit the library's fixed scratch: ndm * nblock * nsub*nchan * 16 bytes
+    if (redigitize_workspace_bytes(g, nblock) > redigitize_static_max_bytes()) return CDMT_ERR_WORKSPACE;
+    plan->last_launches = 0;
+    return check_cuda(launch_redigitize_static(g, d_fb, fb_stride_dm, nblock, qmean, qstd, d_codes, codes_stride_dm,
+                                               d_offset, d_scale, static_cast<cudaStream_t>(cuda_stream),
+                                               &plan->last_launches));
+}
+
 extern "C" int cdmt_redigitize_sums(cdmt_plan *plan, const float *d_fb, long long fb_stride_dm, long long nblock,
                                     double qmean, double qstd, const double *d_segsum, unsigned char *d_codes,
                                     long long codes_stride_dm, float *d_offset, float *d_scale, void *cuda_stream)

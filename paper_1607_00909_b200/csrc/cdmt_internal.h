@@ -63,6 +63,12 @@ cudaError_t launch_redigitize(const Geometry &g, const float *d_fb, long long fb
                               float *d_offset, float *d_scale, void *d_workspace, cudaStream_t st,
                               long long *launches);
 
+// the same with the block sums in a file-scope device array of redigitize_static_max_bytes() bytes (no allocation)
+size_t redigitize_static_max_bytes();
+cudaError_t launch_redigitize_static(const Geometry &g, const float *d_fb, long long fb_stride_dm, long long nblock,
+                                     double qmean, double qstd, unsigned char *d_codes, long long codes_stride_dm,
+                                     float *d_offset, float *d_scale, cudaStream_t st, long long *launches);
+
 cudaError_t launch_block_sums(const Geometry &g, const float *d_fb, long long fb_stride_dm, long long nblock,
                               double *d_segsum, cudaStream_t st, long long *launches);
 cudaError_t launch_stats_quantize(const Geometry &g, const float *d_fb, long long fb_stride_dm, long long nblock,

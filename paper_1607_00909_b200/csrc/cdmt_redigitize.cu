@@ -10,6 +10,7 @@
 // The filterbank is time-major, channel-fastest, so a warp reads 32 adjacent
 // channel groups of one time sample: 512 contiguous bytes with float4 loads (nch % 4 == 0), 128
 // bytes otherwise.  Algorithmic traffic: 4 B + 4 B read and 1 B written per filterbank sample.
+#include <mutex>
 #include <cstdint>
 
 #include "cdmt_internal.h"
@@ -214,6 +215,62 @@ cudaError_t launch_redigitize(const Geometry &g, const float *d_fb, long long fb
     if (e != cudaSuccess) return e;
     return launch_stats_quantize(g, d_fb, fb_stride_dm, nblock, qmean, qstd, segsum, d_codes, codes_stride_dm, d_offset,
                                  d_scale, st, launches);
+}
+
+// ------------------------------------------------------------------------------------------------
+// cdmt_redigitize_static: the same three kernels with the block sums in memory the LIBRARY holds, for
+// callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that
+// forbid cudaMalloc).  The scratch is a file-scope device array of a fixed, modest size: every GPU that
+// loads the library keeps these 4 MiB until the process exits.
+//
+//  * In host code `g_redig_scratch` is only a stand-in for the symbol, NOT a device address: the device
+//    address is looked up with cudaGetSymbolAddress, once per device, with that device current, and it
+//    is that pointer the kernels are given.
+//  * All calls on a device share the array.  It keeps the last call's contents, but nothing has to start
+//    at zero: k_block_sums overwrites every (DM, block, channel) entry that k_channel_stats of the same
+//    call reads.  Calls that overlap on the GPU (two streams, two plans, two host threads) race on it:
+//    the caller must order them (one stream, or events).
+//  * No cudaMalloc, cudaFree, cudaMallocHost or other allocating routine is called.
+// ------------------------------------------------------------------------------------------------
+constexpr size_t REDIG_STATIC_BYTES = (size_t)4 << 20;                       // 262144 (DM, block, channel) entries
+static __device__ __align__(256) unsigned char g_redig_scratch[REDIG_STATIC_BYTES];
+
+constexpr int REDIG_MAX_DEVICES = 64;
+static void *g_redig_scratch_addr[REDIG_MAX_DEVICES];   // device address of the array, per device ordinal
+static std::mutex g_redig_scratch_mutex;
+
+size_t redigitize_static_max_bytes() { return REDIG_STATIC_BYTES; }
+
+// device address of this device's copy of the scratch array (looked up on first use, then remembered)
+static cudaError_t redig_scratch_on_current_device(void **ptr)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= REDIG_MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_redig_scratch_mutex);
+    if (!g_redig_scratch_addr[dev]) {
+        void *p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_redig_scratch);
+        if (e != cudaSuccess) return e;
+        if (!p) return cudaErrorInvalidSymbol;
+        g_redig_scratch_addr[dev] = p;
+    }
+    *ptr = g_redig_scratch_addr[dev];
+    return cudaSuccess;
+}
+
+// The caller (cdmt_api.cu) has checked redigitize_workspace_bytes(g, nblock) <= redigitize_static_max_bytes().
+cudaError_t launch_redigitize_static(const Geometry &g, const float *d_fb, long long fb_stride_dm, long long nblock,
+                                     double qmean, double qstd, unsigned char *d_codes, long long codes_stride_dm,
+                                     float *d_offset, float *d_scale, cudaStream_t st, long long *launches)
+{
+    if (redigitize_workspace_bytes(g, nblock) > REDIG_STATIC_BYTES) return cudaErrorInvalidValue;
+    void *scratch = nullptr;
+    cudaError_t e = redig_scratch_on_current_device(&scratch);
+    if (e != cudaSuccess) return e;
+    return launch_redigitize(g, d_fb, fb_stride_dm, nblock, qmean, qstd, d_codes, codes_stride_dm, d_offset, d_scale,
+                             scratch, st, launches);
 }
 
 }  // namespace cdmt
