@@ -168,6 +168,30 @@ def test_execute_rejects_null_pointers_before_touching_cuda(cdmt):
     assert e.value.status == cdmt.ERR_SIZE
 
 
+def test_redigitize_static_checks_its_limit_on_the_host(cdmt):
+    """cdmt_redigitize_static (no workspace, no allocation): null pointers, bad targets and batches beyond the
+    library's fixed 4 MiB scratch are refused with a status before anything touches CUDA."""
+    assert cdmt.cdmt_redigitize_static_max_bytes() == 4 << 20
+    fcen = 120.0 + synth.BW_MHZ * (np.arange(40) + 0.5)
+    p = cdmt.cdmt_plan_create(40, fcen, synth.BW_MHZ, 8192, 7936, 16, 2, np.arange(64.0))     # Vd = 8, 640 channels
+    plane = 40 * 8 * 640
+    # 64 DMs x 40 blocks x 640 channels x 16 bytes = 26 MB of block sums: more than the static array holds
+    assert cdmt.cdmt_redigitize_workspace_bytes(p, 40) == 64 * 40 * 640 * 16
+    with pytest.raises(cdmt.CdmtError) as e:
+        cdmt.cdmt_redigitize_static(p, 256, plane, 40, 64.0, 16.0, 256, plane, 256, 256, stream=0)
+    assert e.value.status == cdmt.ERR_WORKSPACE
+    for bad in [dict(d_fb=0), dict(d_codes=0), dict(d_offset=0), dict(d_scale=0), dict(d_fb=258), dict(qstd=0.0)]:
+        a = dict(d_fb=256, d_codes=256, d_offset=256, d_scale=256, qstd=16.0)
+        a.update(bad)
+        with pytest.raises(cdmt.CdmtError) as e:
+            cdmt.cdmt_redigitize_static(p, a["d_fb"], 8 * 640, 1, 64.0, a["qstd"], a["d_codes"], 8 * 640,
+                                        a["d_offset"], a["d_scale"], stream=0)
+        assert e.value.status == cdmt.ERR_ARG, bad
+    with pytest.raises(cdmt.CdmtError) as e:
+        cdmt.cdmt_redigitize_static(p, 256, 8 * 640 - 1, 1, 64.0, 16.0, 256, 8 * 640, 256, 256, stream=0)  # short plane stride
+    assert e.value.status == cdmt.ERR_SIZE
+
+
 def test_sweep_seconds_eq2_against_paper_values(cdmt):
     vals = {}
     for line in open(os.path.join(ROOT, "tests", "golden", "paper_values.txt")):
